@@ -1,0 +1,326 @@
+#!/usr/bin/env python
+"""bench.py -- MLUPS of the full LB+FD step and achieved HBM bandwidth of the LB kernel.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config 3] [--precision fp32s|fp64|fp32u] [--size NX NY NZ]
+
+Workload (default): BASELINE.json configs[3] -- two skyrmion tubes in Poiseuille flow on
+256x256x64, FD/LB ratio r = 10, shifted FP32 (the configuration north_star's target is quoted on).
+One bench "step" is one pass over every row of the hot path: r LB steps (collide+stream+force),
+then the velocity store, predictor, corrector and force update.  MLUPS = fluid cells x LB steps /
+seconds / 1e6 (reading G21).
+
+Prints ONE JSON line (rank 0).  Multi-GPU: the path is not sharded ("replicas only"):
+--gpus N runs N independent replicas, one per rank, and reports their summed throughput.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+PRECISIONS = {"fp64": 0, "fp32s": 1, "fp32u": 2, "fp64u": 3}
+DTYPE = {0: "f64", 1: "f32", 2: "f32", 3: "f64"}
+METRIC = "MLUPS (LB+FD step)"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--precision", default="fp32s", choices=sorted(PRECISIONS))
+    ap.add_argument("--size", type=int, nargs=3, default=None, help="configs[4] grid (nx ny nz)")
+    ap.add_argument("--options", type=int, default=0, help="nh_set_options bits (kernel variants)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload(args):
+    import nh_inputs as I
+    over = {}
+    if args.config == 4 and args.size:
+        over["size"] = tuple(args.size)
+    p = I.config(args.config, **over)
+    d = p.pop("director")
+    p.pop("steps")
+    name = {0: "configs[0] tiny channel", 1: "configs[1] single skyrmion tube", 2: "configs[2] precision sweep domain",
+            3: "configs[3] two skyrmion tubes in Poiseuille flow", 4: "configs[4] skyrmion lattice"}[args.config]
+    desc = {"workload": "%s %dx%dx%d" % (name, p["nx"], p["ny"], p["nz"]), "grid": [p["nx"], p["ny"], p["nz"]],
+            "fd_ratio": p["fd_ratio"], "tau": p["tau"], "K": p["K"], "pitch": p["pitch"], "xi": p["xi"],
+            "g_x": p["g"][0], "precision": args.precision}
+    return p, d, desc
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(precision):
+    """DRAM bytes per LB launch from the committed ncu --set full capture, or None."""
+    path = os.path.join(ROOT, "profiles", "lb_traffic.json")
+    if not os.path.exists(path):
+        return None
+    try:
+        rec = json.load(open(path))
+        return rec.get(str(precision), {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks line of B200_PROFILING.md, sampled during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            out = self.proc.communicate(timeout=5)[0]
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2])); power.append(float(c[3]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": max(power)}
+
+
+def run_reference(args):
+    """The oracle, as it stands, on the host cores (tier contract: the reference arm)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import Oracle, num_threads
+    p, d, desc = workload(args)
+    o = Oracle(**dict(p, precision=PRECISIONS[args.precision]))
+    o.set_director(d)
+    nf = p["nx"] * p["ny"] * (p["nz"] - 2)
+    o.step(args.warmup)
+    t0 = time.perf_counter()
+    o.step(args.steps)
+    dt = time.perf_counter() - t0
+    mlups = nf * args.steps / dt / 1e6
+    sample = ("each step = one LB step of the full grid, the FD update firing on every %d-th "
+              "(%d steps timed)" % (p["fd_ratio"], args.steps))
+    line = {"impl": "reference", "metric": METRIC, "value": mlups, "unit": "MLUPS", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": desc,
+            "cpu_baseline": {"value": mlups, "unit": "MLUPS", "cores": num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": mlups, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def cpu_baseline(p, d, precision):
+    from oracle import Oracle, num_threads
+    o = Oracle(**dict(p, precision=precision))
+    o.set_director(d)
+    r = max(1, p["fd_ratio"])
+    nf = p["nx"] * p["ny"] * (p["nz"] - 2)
+    # bounded sample: whole FD periods of the same workload, about 10-30 s of CPU work; the first
+    # period sizes the sample, the rest is what is timed
+    t0 = time.perf_counter()
+    o.step(r)
+    first = time.perf_counter() - t0
+    periods = max(1, min(200, int(12.0 / max(first, 1e-3))))
+    t0 = time.perf_counter()
+    o.step(periods * r)
+    dt = time.perf_counter() - t0
+    return {"value": nf * periods * r / dt / 1e6, "unit": "MLUPS", "cores": num_threads(), "kind": "oracle",
+            "sample": "%d FD period(s) = %d LB steps + %d FD update(s) of the same %dx%dx%d workload, %.1f s"
+                      % (periods, periods * r, periods, p["nx"], p["ny"], p["nz"], dt)}
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    import paper_2503_06610_b200 as nh
+    from paper_2503_06610_b200 import build as nh_build
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl ours needs a CUDA device (there is no CPU path)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        nh_build.build()
+    if world > 1:
+        dist.barrier()
+
+    p, d, desc = workload(args)
+    prec = PRECISIONS[args.precision]
+    r = max(1, p["fd_ratio"])
+    nf = p["nx"] * p["ny"] * (p["nz"] - 2)
+    N = p["nx"] * p["ny"] * p["nz"]
+    word = 8 if prec in (0, 3) else 4
+    lat = nh.Lattice(device="cuda:%d" % local, **dict(p, precision=prec))
+    d_pinned = torch.from_numpy(d).pin_memory()
+    lat.set_director(d_pinned)
+    base_opt = args.options
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        ev0.record()
+        fn()
+        ev1.record()
+        barrier()
+        ms = ev0.elapsed_time(ev1)
+        if world > 1:
+            t = torch.tensor([ms], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps ----------------------------
+    lat.set_options(base_opt)
+    for _ in range(args.warmup):
+        lat.step(r)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = lat.launch_count
+    ms = timed(lambda: [lat.step(r) for _ in range(args.steps)])
+    launches = lat.launch_count - l0
+    clocks = sampler.stop() if rank == 0 else None
+    mlups = world * nf * r * args.steps / (ms * 1e-3) / 1e6
+
+    # ---- second pass of the same K steps with a CUDA-event pair around every launch ---------------
+    lat.set_options(base_opt | nh.OPT_TIMING)
+    barrier()
+    for _ in range(args.steps):
+        lat.step(r)
+    kt = {k: lat.kernel_time(k) for k in nh.KERNEL_CLASSES}
+    lat.set_options(base_opt)
+    lb_ms, lb_n = kt["lb"]
+    lb_avg = lb_ms / max(lb_n, 1)
+    total_k = sum(v[0] for v in kt.values())
+    peak, peak_src = peaks()
+    alg_bytes = 41 * word * nf          # 19 read + 19 write + 3 (F^LC) words per fluid cell
+    achieved = alg_bytes / (lb_avg * 1e-3) / 1e9 if lb_avg > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": "lb_step (collide+stream+force)", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(prec),
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
+                "avg_launch_ms": lb_avg, "launches_timed": lb_n, "share_of_step": lb_ms / total_k if total_k else None,
+                "kernel_ms": {k: round(v[0], 4) for k, v in kt.items()},
+                "full_step_bytes_per_cell": (41 + 30.0 / r) * word,
+                "full_step_achieved_gbs": (41 + 30.0 / r) * word * nf * r * args.steps / (ms * 1e-3) / 1e9,
+                "timed": "second pass of the same K steps with per-launch CUDA events on the launch stream"}
+
+    # ---- end to end through the C ABI with host buffers --------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        out = {"u": torch.empty((3, p["nz"], p["ny"], p["nx"]), dtype=torch.float64).pin_memory(),
+               "n": torch.empty((3, p["nz"], p["ny"], p["nx"]), dtype=torch.float64).pin_memory()}
+
+        def job():
+            lat.set_director(d_pinned)                      # H2D 3N doubles
+            for _ in range(args.steps):
+                lat.step(r)
+            lat.get_fields(out=out, which=("u", "n"))       # D2H 6N doubles
+
+        job()
+        ms_job = timed(job)
+
+        def every():
+            for _ in range(3):
+                lat.set_director(d_pinned)
+                lat.step(r)
+                lat.get_fields(out=out, which=("u", "n"))
+
+        ms_every = timed(every)
+        e2e = {"value": world * nf * r * args.steps / (ms_job * 1e-3) / 1e6, "unit": "MLUPS",
+               "h2d_bytes_per_step": 24 * N / args.steps, "d2h_bytes_per_step": 48 * N / args.steps,
+               "what": "one job = nh_set_director(pinned host n) + K steps + nh_get_fields(u, n -> pinned host), "
+                       "all inside the timed region; bytes are the job's copies divided by K",
+               "copies_every_step": {"value": world * nf * r * 3 / (ms_every * 1e-3) / 1e6, "unit": "MLUPS",
+                                     "h2d_bytes_per_step": 24 * N, "d2h_bytes_per_step": 48 * N}}
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    line = {"metric": METRIC, "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": DTYPE[prec], "data": "synthetic",
+            "config": dict(desc, lb_steps_per_step=r, fluid_cells=nf, parallelism="replicas x%d" % world,
+                           l2="populations (2 x %.0f MB) exceed the 126 MB L2; no flush needed" % (19 * N * word / 1e6),
+                           options=base_opt),
+            "clocks": clocks, "gpu_launches": launches, "roofline": roofline}
+    if e2e is not None:
+        line["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(p, d, prec)
+    print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

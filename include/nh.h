@@ -1,0 +1,125 @@
+/* nh.h -- C ABI of the B200 (sm_100a) nematohydrodynamics hot path.
+ *
+ * One LB+FD time step of the hybrid solver of arXiv 2503.06610 ("Efficient single-precision
+ * simulations of nematohydrodynamics"), in the reduced form BASELINE.json's north_star names:
+ *
+ *   flow     : D3Q19 single-relaxation-time lattice Boltzmann with Guo forcing on the SHIFTED
+ *              populations f_i - w_i                      PAPER.md:118-166, Eqs. 14-23 (Sec. II.C)
+ *              half-way bounce-back at the two plates     PAPER.md:141;  periodic x, y PAPER.md:225
+ *   director : d_t n = h/gamma1 + xi n.D - (u.grad) n + W.n, projected perpendicular to n,
+ *              predictor-corrector, renormalised           PAPER.md:77 (Eq. 9), 105-112 (Sec. II.B)
+ *              h = K lap n - 2 K q0 curl n  (one-constant Frank energy with chiral term)
+ *                                                          PAPER.md:70-73, 81 (Eqs. 7-8, 10)
+ *   force    : F^LC_a = d_b sigma_ab,  sigma = elastic (Ericksen) stress
+ *                                                          PAPER.md:66 (Eq. 6), 97 (Eq. 12, last term)
+ *   schedule : LB every step; director + force after every r-th step with Delta t_FD = r
+ *                                                          PAPER.md:191-207 (Sec. II.D, Fig. 1)
+ *
+ * Every step of that path runs in hand-written CUDA kernels (paper_2503_06610_b200/csrc).  There
+ * is no CPU fallback: without a CUDA device every compute entry returns NH_ECUDA.
+ *
+ * Conventions
+ *   - Return value: 0 (NH_OK) or a negative code; the message is in nh_last_error() (per thread).
+ *     No exception or abort crosses this boundary.
+ *   - Fields are arrays [component][z][y][x], x fastest, N = nx*ny*nz cells.  Layers z = 0 and
+ *     z = nz-1 are the solid plates (wall half-way between layers 0|1 and nz-2|nz-1); the fluid is
+ *     z = 1..nz-2.  On the plates rho = 1, u = 0, F^LC = 0 and n = z_hat are returned.
+ *   - Every HOST array is FP64 whatever the device precision; conversion happens on the device.
+ *   - Ownership: the caller owns all host arrays and the device workspace and keeps the workspace
+ *     alive until nh_free.  The library owns only the handle.
+ *   - All device work is enqueued on the stream given to nh_init_lattice.  nh_set_director and
+ *     nh_get_fields synchronise that stream before returning; nh_step does not.
+ */
+#ifndef NH_H
+#define NH_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NH_OK       0
+#define NH_EINVAL  -1   /* null pointer, bad size or parameter                      */
+#define NH_ENOMEM  -2   /* workspace smaller than nh_workspace_bytes()              */
+#define NH_ECUDA   -3   /* a CUDA call failed (including: no device)                */
+
+/* precision */
+#define NH_FP64_SHIFTED    0   /* Eqs. 19-23 in double                                */
+#define NH_FP32_SHIFTED    1   /* Eqs. 19-23 in float: the paper's method            */
+#define NH_FP32_UNSHIFTED  2   /* Eqs. 14-17 in float: the comparison PAPER.md:235   */
+#define NH_FP64_UNSHIFTED  3   /* Eqs. 14-17 in double                                */
+
+typedef struct nh_lattice nh_lattice;   /* opaque */
+
+typedef struct {
+  int    nx, ny, nz;   /* grid; nz counts the two plate layers; nx, ny >= 1, nz >= 3            */
+  double tau;          /* SRT relaxation time, > 0.5; nu = (tau - 1/2)/3 */
+  double K;            /* one-constant Frank modulus, >= 0 */
+  double pitch;        /* cholesteric pitch P in cells, q0 = 2 pi/P; <= 0: q0 = 0 PAPER.md:73  */
+  double xi;           /* flow-alignment parameter = -gamma2/gamma1  */
+  double gamma1;       /* rotational viscosity, > 0  */
+  double g[3];         /* body acceleration; the force on the fluid is rho g  */
+  int    anchoring;    /* 0 = infinite homeotropic at both plates (only value built) PAPER.md:103 */
+  double W0;           /* bulk anchoring strength; must be 0 (not built) */
+  int    fd_ratio;     /* default r = Delta t_FD / Delta t_LB, >= 0 */
+  int    precision;    /* NH_FP64_SHIFTED .. NH_FP64_UNSHIFTED */
+  int    coupling;     /* bit0: F^LC acts on the flow; bit1: the flow acts on n   (3 = paper)  */
+} nh_params;
+
+/* Bytes of device memory the lattice needs for these parameters (0 if they are invalid).
+ * Layout: two population buffers [19][N], n, n^P, n', u, F^LC [3][N]
+ * in the device precision, one FP64 staging buffer [3][N], each 256-byte aligned. */
+size_t nh_workspace_bytes(const nh_params* p);
+
+/* Create a lattice in `dev_workspace` (DEVICE pointer, 256-byte aligned, >= nh_workspace_bytes).
+ * `cuda_stream` is a cudaStream_t (NULL = legacy default stream).  State after the call: t = 0,
+ * rho = 1, u = 0 (shifted populations 0, Eq. 19), n = z_hat, F^LC = 0.  PAPER.md:193-199. */
+int nh_init_lattice(const nh_params* p, void* dev_workspace, size_t bytes, void* cuda_stream,
+                    nh_lattice** out);
+
+/* Set the director from a HOST array [3][nz][ny][nx] (FP64).  Each vector is normalised, the plate
+ * layers are overwritten with z_hat, n^P := n and F^LC is computed from it
+ * (Eq. 12; reading G9).  Populations and t are untouched.  NH_EINVAL if a vector has
+ * zero or non-finite length (checked on the device; the lattice is then unchanged). */
+int nh_set_director(nh_lattice* L, const double* n_host);
+
+/* Advance n_lb lattice-Boltzmann steps.  r = n_fd (n_fd < 0: params.fd_ratio; 0: director and
+ * force frozen).  After each LB step t <- t+1 and, if r > 0 and t mod r == 0, the director
+ * predictor-corrector and the force update run with Delta t_FD = r.
+ * Asynchronous on the lattice's stream. */
+int nh_step(nh_lattice* L, int n_lb, int n_fd);
+
+/* Copy fields to HOST arrays (FP64); any pointer may be NULL.  rho [N] and u [3][N] are Eqs. 20-21
+ * on the current (post-streaming) populations with the current force; n [3][N]; F_lc [3][N]. */
+int nh_get_fields(nh_lattice* L, double* rho, double* u, double* n, double* F_lc);
+
+/* Number of completed LB steps (-1 for a null handle). */
+long nh_time(const nh_lattice* L);
+
+/* Number of kernels this lattice has launched so far (bench.py's gpu_launches). */
+long nh_launch_count(const nh_lattice* L);
+
+/* Options (results do not depend on them):
+ *   bit0 NH_OPT_GRAPH     replay nh_step through CUDA graphs (launch-bound small grids)
+ *   bit1 NH_OPT_TIMING    bracket every kernel launch with a CUDA-event pair on the lattice's stream
+ *   bit2 NH_OPT_FD_DIRECT use the one-thread-per-cell FD kernels instead of the tiled ones
+ *   bit3 NH_OPT_LB_SCALAR use the one-cell-per-thread LB kernel instead of the wide one
+ * Setting options resets the timing accumulators. */
+#define NH_OPT_GRAPH      1
+#define NH_OPT_TIMING     2
+#define NH_OPT_FD_DIRECT  4
+#define NH_OPT_LB_SCALAR  8
+int nh_set_options(nh_lattice* L, int options);
+
+/* Accumulated CUDA-event time (ms) and number of launches of one kernel class since the last
+ * nh_set_options; synchronises the stream.  Time is only accumulated while NH_OPT_TIMING is set.
+ * which: 0 = LB collide+stream, 1 = velocity (moments, u store), 2 = predictor, 3 = corrector,
+ *        4 = force, 5 = everything else (conversions, initialisation). */
+int nh_kernel_time(nh_lattice* L, int which, double* ms_total, long* launches);
+
+void nh_free(nh_lattice* L);
+const char* nh_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,429 @@
+// nh_api.cu -- host side of the C ABI declared in include/nh.h: workspace carving, the LB/FD
+// schedule of Fig. 1, kernel dispatch over the precision variants, CUDA-event
+// timing per kernel class.  No arithmetic of the method lives here: every step runs in the
+// kernels of nh_lb.cuh / nh_fd.cuh.
+#include "../../include/nh.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "nh_fd.cuh"
+#include "nh_lb.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+int fail(int code, const std::string& m) { g_err = m; return code; }
+int cuda_fail(cudaError_t e, const char* what) {
+  g_err = std::string(what) + ": " + cudaGetErrorString(e);
+  return NH_ECUDA;
+}
+#define NH_CUDA(call)                                   \
+  do {                                                  \
+    cudaError_t e_ = (call);                            \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+  } while (0)
+
+constexpr size_t ALIGN = 256;
+size_t align_up(size_t b) { return (b + ALIGN - 1) / ALIGN * ALIGN; }
+
+const char* check_params(const nh_params* p) {
+  if (!p) return "null params";
+  if (p->nx < 1 || p->ny < 1 || p->nz < 3) return "need nx, ny >= 1 and nz >= 3";
+  const double cells = (double)p->nx * p->ny * p->nz;
+  if (cells * 19.0 >= 2147483648.0) return "grid too large: 19*nx*ny*nz must stay below 2^31";
+  if (!(p->tau > 0.5) || !std::isfinite(p->tau)) return "tau must be > 0.5";
+  if (!(p->gamma1 > 0.0) || !std::isfinite(p->gamma1)) return "gamma1 must be > 0";
+  if (!(p->K >= 0.0) || !std::isfinite(p->K)) return "K must be >= 0";
+  if (!std::isfinite(p->pitch) || !std::isfinite(p->xi)) return "pitch and xi must be finite";
+  if (!std::isfinite(p->g[0]) || !std::isfinite(p->g[1]) || !std::isfinite(p->g[2])) return "g must be finite";
+  if (p->fd_ratio < 0) return "fd_ratio must be >= 0";
+  if (p->precision < 0 || p->precision > 3) return "precision must be 0..3";
+  if (p->anchoring != 0 || p->W0 != 0.0) return "only anchoring = 0 and W0 = 0 are built";
+  if (p->coupling < 0 || p->coupling > 3) return "coupling must be 0..3";
+  return nullptr;
+}
+
+size_t word_of(int precision) {
+  return (precision == NH_FP64_SHIFTED || precision == NH_FP64_UNSHIFTED) ? 8 : 4;
+}
+
+enum KernelClass { KC_LB = 0, KC_VEL = 1, KC_PRED = 2, KC_CORR = 3, KC_FORCE = 4, KC_OTHER = 5, KC_COUNT = 6 };
+
+}  // namespace
+
+struct nh_lattice {
+  nh_params p;
+  nh::Geom G;
+  double q0;
+  cudaStream_t stream;
+  long t;
+  long launches;
+  int options;
+  // device pointers into the caller's workspace (type-erased; word = 4 or 8 bytes)
+  void* f[2];       // population ping-pong; f[cur] is what the next LB step gathers from
+  int cur;
+  void* n[2];       // director ping-pong; n[ncur] is the current director
+  int ncur;
+  void* nP;
+  void* u;
+  void* F;
+  double* stage;    // FP64 staging [3][N]
+  int* flag;
+  // per-class CUDA-event timing (option bit1)
+  struct Pair { cudaEvent_t a, b; int cls; };
+  std::vector<Pair> pool;
+  size_t used;
+  double ms[KC_COUNT];
+  long cnt[KC_COUNT];
+};
+
+namespace {
+
+constexpr int BLOCK = 256;
+unsigned blocks_for(size_t n) { return (unsigned)((n + BLOCK - 1) / BLOCK); }
+
+int drain_events(nh_lattice* L) {
+  if (L->used == 0) return NH_OK;
+  NH_CUDA(cudaStreamSynchronize(L->stream));
+  for (size_t i = 0; i < L->used; ++i) {
+    float ms = 0.f;
+    NH_CUDA(cudaEventElapsedTime(&ms, L->pool[i].a, L->pool[i].b));
+    L->ms[L->pool[i].cls] += ms;
+  }
+  L->used = 0;
+  return NH_OK;
+}
+
+// Counts one launch of class `cls` and, with NH_OPT_TIMING, brackets it with an event pair:
+// construct before the launch; end() (or the destructor) records the closing event after it.
+struct Bracket {
+  nh_lattice* L;
+  int slot;
+  int rc;
+  ~Bracket() { end(); }
+  Bracket(nh_lattice* L_, int cls) : L(L_), slot(-1), rc(NH_OK) {
+    L->launches += 1;
+    L->cnt[cls] += 1;
+    if (!(L->options & 2)) return;
+    if (L->used == L->pool.size()) {
+      if (L->pool.size() >= 4096) { rc = drain_events(L); if (rc) return; }
+      else {
+        nh_lattice::Pair pr;
+        if (cudaEventCreate(&pr.a) != cudaSuccess || cudaEventCreate(&pr.b) != cudaSuccess) {
+          rc = fail(NH_ECUDA, "cudaEventCreate failed");
+          return;
+        }
+        L->pool.push_back(pr);
+      }
+    }
+    slot = (int)L->used++;
+    L->pool[slot].cls = cls;
+    cudaEventRecord(L->pool[slot].a, L->stream);
+  }
+  void end() {
+    if (slot >= 0) cudaEventRecord(L->pool[slot].b, L->stream);
+    slot = -1;
+  }
+};
+
+template <typename T>
+nh::LbConst<T> lb_const(const nh_lattice* L) {
+  nh::LbConst<T> C;
+  C.omega = (T)(1.0 / L->p.tau);
+  C.somega = (T)(1.0 - 1.0 / (2.0 * L->p.tau));
+  C.gx = (T)L->p.g[0]; C.gy = (T)L->p.g[1]; C.gz = (T)L->p.g[2];
+  C.use_flc = L->p.coupling & 1;
+  return C;
+}
+template <typename T>
+nh::FdConst<T> fd_const(const nh_lattice* L, int r) {
+  nh::FdConst<T> C;
+  C.K = (T)L->p.K;
+  C.Kq0 = (T)(L->p.K * L->q0);
+  C.inv_gamma1 = (T)(1.0 / L->p.gamma1);
+  C.xi = (T)L->p.xi;
+  C.dt = (T)r;
+  return C;
+}
+
+// ---- typed launchers ----------------------------------------------------------------------------
+template <typename T, bool SH>
+int launch_lb(nh_lattice* L) {
+  Bracket br(L, KC_LB);
+  if (br.rc) return br.rc;
+  nh::lb_step_kernel<T, SH><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
+      (const T*)L->f[L->cur], (T*)L->f[L->cur ^ 1], (const T*)L->F, L->G, lb_const<T>(L));
+  br.end();
+  return NH_OK;
+}
+template <typename T, bool SH>
+int launch_velocity(nh_lattice* L) {
+  Bracket br(L, KC_VEL);
+  if (br.rc) return br.rc;
+  nh::velocity_kernel<T, SH><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
+      (const T*)L->f[L->cur], (const T*)L->F, (T*)L->u, L->G, lb_const<T>(L));
+  br.end();
+  return NH_OK;
+}
+template <typename T>
+int launch_force(nh_lattice* L) {
+  Bracket br(L, KC_FORCE);
+  if (br.rc) return br.rc;
+  nh::force_direct_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
+      (const T*)L->n[L->ncur], (T*)L->F, L->G, fd_const<T>(L, 1));
+  br.end();
+  return NH_OK;
+}
+template <typename T>
+int launch_director(nh_lattice* L, int r) {
+  const int with_flow = (L->p.coupling & 2) ? 1 : 0;
+  const nh::FdConst<T> C = fd_const<T>(L, r);
+  {
+    Bracket br(L, KC_PRED);
+    if (br.rc) return br.rc;
+    nh::predictor_direct_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
+        (const T*)L->n[L->ncur], (const T*)L->u, (T*)L->nP, L->G, C, with_flow);
+    br.end();
+  }
+  {
+    Bracket br(L, KC_CORR);
+    if (br.rc) return br.rc;
+    nh::corrector_direct_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
+        (const T*)L->n[L->ncur], (const T*)L->nP, (const T*)L->u, (T*)L->n[L->ncur ^ 1], L->G, C, with_flow);
+    br.end();
+  }
+  L->ncur ^= 1;
+  return NH_OK;
+}
+
+template <typename T, bool SH>
+int step_typed(nh_lattice* L, int n_lb, int r) {
+  for (int s = 0; s < n_lb; ++s) {
+    int rc = launch_lb<T, SH>(L);
+    if (rc) return rc;
+    L->cur ^= 1;
+    L->t += 1;
+    if (r > 0 && L->t % r == 0) {
+      if (L->p.coupling & 2) { rc = launch_velocity<T, SH>(L); if (rc) return rc; }
+      rc = launch_director<T>(L, r); if (rc) return rc;
+      rc = launch_force<T>(L); if (rc) return rc;
+    }
+  }
+  NH_CUDA(cudaGetLastError());
+  return NH_OK;
+}
+
+template <typename T, bool SH>
+int init_typed(nh_lattice* L) {
+  const size_t N = L->G.N;
+  for (int b = 0; b < 2; ++b) {
+    Bracket br(L, KC_OTHER);
+    nh::rest_kernel<T, SH><<<blocks_for(N), BLOCK, 0, L->stream>>>((T*)L->f[b], L->G);
+  }
+  NH_CUDA(cudaMemsetAsync(L->u, 0, 3 * N * sizeof(T), L->stream));
+  NH_CUDA(cudaMemsetAsync(L->F, 0, 3 * N * sizeof(T), L->stream));
+  // n = z_hat everywhere: stage := (0, 0, 1), then the same store kernel
+  NH_CUDA(cudaMemsetAsync(L->stage, 0, 2 * N * sizeof(double), L->stream));
+  {
+    Bracket br(L, KC_OTHER);
+    nh::fill_f64_kernel<<<blocks_for(N), BLOCK, 0, L->stream>>>(L->stage + 2 * N, 1.0, N);
+  }
+  {
+    Bracket br(L, KC_OTHER);
+    nh::store_director_kernel<T><<<blocks_for(N), BLOCK, 0, L->stream>>>(
+        L->stage, (T*)L->n[0], (T*)L->nP, (T*)L->n[1], L->G);
+  }
+  NH_CUDA(cudaGetLastError());
+  NH_CUDA(cudaStreamSynchronize(L->stream));
+  return NH_OK;
+}
+
+template <typename T>
+int set_director_typed(nh_lattice* L) {
+  const size_t N = L->G.N;
+  {
+    Bracket br(L, KC_OTHER);
+    nh::store_director_kernel<T><<<blocks_for(N), BLOCK, 0, L->stream>>>(
+        L->stage, (T*)L->n[L->ncur], (T*)L->nP, (T*)L->n[L->ncur ^ 1], L->G);
+  }
+  return launch_force<T>(L);  // reading G9: force from the initial director
+}
+
+template <typename T, bool SH>
+int get_fields_typed(nh_lattice* L, double* rho, double* u, double* n, double* F) {
+  const size_t N = L->G.N;
+  if (rho || u) {
+    // stage = [ux uy uz]; rho goes through the first N doubles in a second pass
+    if (u) {
+      Bracket br(L, KC_OTHER);
+      nh::fields_kernel<T, SH><<<blocks_for(N), BLOCK, 0, L->stream>>>(
+          (const T*)L->f[L->cur], (const T*)L->F, nullptr, L->stage, L->G, lb_const<T>(L));
+      br.end();
+      NH_CUDA(cudaMemcpyAsync(u, L->stage, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
+    }
+    if (rho) {
+      Bracket br(L, KC_OTHER);
+      nh::fields_kernel<T, SH><<<blocks_for(N), BLOCK, 0, L->stream>>>(
+          (const T*)L->f[L->cur], (const T*)L->F, L->stage, nullptr, L->G, lb_const<T>(L));
+      br.end();
+      NH_CUDA(cudaMemcpyAsync(rho, L->stage, N * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
+    }
+  }
+  const void* src[2] = {L->n[L->ncur], L->F};
+  double* dst[2] = {n, F};
+  for (int k = 0; k < 2; ++k) {
+    if (!dst[k]) continue;
+    Bracket br(L, KC_OTHER);
+    nh::widen3_kernel<T><<<blocks_for(3 * N), BLOCK, 0, L->stream>>>((const T*)src[k], L->stage, 3 * N);
+    br.end();
+    NH_CUDA(cudaMemcpyAsync(dst[k], L->stage, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
+  }
+  NH_CUDA(cudaGetLastError());
+  NH_CUDA(cudaStreamSynchronize(L->stream));
+  return NH_OK;
+}
+
+#define NH_DISPATCH(L, CALL_F64S, CALL_F32S, CALL_F32U, CALL_F64U) \
+  switch ((L)->p.precision) {                                      \
+    case NH_FP64_SHIFTED: return CALL_F64S;                        \
+    case NH_FP32_SHIFTED: return CALL_F32S;                        \
+    case NH_FP32_UNSHIFTED: return CALL_F32U;                      \
+    default: return CALL_F64U;                                     \
+  }
+
+}  // namespace
+
+extern "C" {
+
+const char* nh_last_error(void) { return g_err.c_str(); }
+
+size_t nh_workspace_bytes(const nh_params* p) {
+  if (check_params(p)) return 0;
+  const size_t N = (size_t)p->nx * p->ny * p->nz;
+  const size_t w = word_of(p->precision);
+  size_t b = 0;
+  b += 2 * align_up(19 * N * w);   // populations A, B
+  b += 5 * align_up(3 * N * w);    // n[0], n[1], nP, u, F
+  b += align_up(3 * N * sizeof(double));  // staging
+  b += ALIGN;                      // flag
+  return b;
+}
+
+int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_stream, nh_lattice** out) {
+  if (!out) return fail(NH_EINVAL, "null out pointer");
+  *out = nullptr;
+  const char* bad = check_params(p);
+  if (bad) return fail(NH_EINVAL, bad);
+  if (!ws) return fail(NH_EINVAL, "null workspace");
+  if ((size_t)ws % ALIGN) return fail(NH_EINVAL, "workspace must be 256-byte aligned");
+  if (bytes < nh_workspace_bytes(p)) return fail(NH_ENOMEM, "workspace smaller than nh_workspace_bytes()");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(NH_ECUDA, "no CUDA device: this library has no CPU path");
+  }
+  nh_lattice* L = new (std::nothrow) nh_lattice();
+  if (!L) return fail(NH_ENOMEM, "out of host memory");
+  L->p = *p;
+  L->G.nx = p->nx; L->G.ny = p->ny; L->G.nz = p->nz;
+  L->G.plane = (unsigned)p->nx * p->ny;
+  L->G.nfluid = L->G.plane * (unsigned)(p->nz - 2);
+  L->G.N = (size_t)L->G.plane * p->nz;
+  L->q0 = p->pitch > 0.0 ? 2.0 * M_PI / p->pitch : 0.0;
+  L->stream = (cudaStream_t)cuda_stream;
+  L->t = 0; L->launches = 0; L->options = 0; L->cur = 0; L->ncur = 0; L->used = 0;
+  for (int k = 0; k < KC_COUNT; ++k) { L->ms[k] = 0.0; L->cnt[k] = 0; }
+  const size_t N = L->G.N, w = word_of(p->precision);
+  char* base = (char*)ws;
+  auto take = [&](size_t b) { char* q = base; base += align_up(b); return (void*)q; };
+  L->f[0] = take(19 * N * w); L->f[1] = take(19 * N * w);
+  L->n[0] = take(3 * N * w); L->n[1] = take(3 * N * w);
+  L->nP = take(3 * N * w); L->u = take(3 * N * w); L->F = take(3 * N * w);
+  L->stage = (double*)take(3 * N * sizeof(double));
+  L->flag = (int*)take(sizeof(int));
+  int rc;
+  switch (p->precision) {
+    case NH_FP64_SHIFTED: rc = init_typed<double, true>(L); break;
+    case NH_FP32_SHIFTED: rc = init_typed<float, true>(L); break;
+    case NH_FP32_UNSHIFTED: rc = init_typed<float, false>(L); break;
+    default: rc = init_typed<double, false>(L); break;
+  }
+  if (rc) { delete L; return rc; }
+  *out = L;
+  return NH_OK;
+}
+
+int nh_set_director(nh_lattice* L, const double* n_host) {
+  if (!L || !n_host) return fail(NH_EINVAL, "null pointer");
+  const size_t N = L->G.N;
+  NH_CUDA(cudaMemcpyAsync(L->stage, n_host, 3 * N * sizeof(double), cudaMemcpyHostToDevice, L->stream));
+  NH_CUDA(cudaMemsetAsync(L->flag, 0, sizeof(int), L->stream));
+  {
+    Bracket br(L, KC_OTHER);
+    nh::check_director_kernel<<<blocks_for(N), BLOCK, 0, L->stream>>>(L->stage, N, L->flag);
+  }
+  int flag = 0;
+  NH_CUDA(cudaMemcpyAsync(&flag, L->flag, sizeof(int), cudaMemcpyDeviceToHost, L->stream));
+  NH_CUDA(cudaStreamSynchronize(L->stream));
+  if (flag) return fail(NH_EINVAL, "zero-length or non-finite director vector");
+  int rc;
+  if (word_of(L->p.precision) == 8) rc = set_director_typed<double>(L);
+  else rc = set_director_typed<float>(L);
+  if (rc) return rc;
+  NH_CUDA(cudaGetLastError());
+  NH_CUDA(cudaStreamSynchronize(L->stream));
+  return NH_OK;
+}
+
+int nh_step(nh_lattice* L, int n_lb, int n_fd) {
+  if (!L) return fail(NH_EINVAL, "null handle");
+  if (n_lb < 0) return fail(NH_EINVAL, "n_lb must be >= 0");
+  const int r = n_fd < 0 ? L->p.fd_ratio : n_fd;
+  NH_DISPATCH(L, (step_typed<double, true>(L, n_lb, r)), (step_typed<float, true>(L, n_lb, r)),
+              (step_typed<float, false>(L, n_lb, r)), (step_typed<double, false>(L, n_lb, r)));
+}
+
+int nh_get_fields(nh_lattice* L, double* rho, double* u, double* n, double* F_lc) {
+  if (!L) return fail(NH_EINVAL, "null handle");
+  NH_DISPATCH(L, (get_fields_typed<double, true>(L, rho, u, n, F_lc)),
+              (get_fields_typed<float, true>(L, rho, u, n, F_lc)),
+              (get_fields_typed<float, false>(L, rho, u, n, F_lc)),
+              (get_fields_typed<double, false>(L, rho, u, n, F_lc)));
+}
+
+long nh_time(const nh_lattice* L) { return L ? L->t : -1; }
+long nh_launch_count(const nh_lattice* L) { return L ? L->launches : -1; }
+
+int nh_set_options(nh_lattice* L, int options) {
+  if (!L) return fail(NH_EINVAL, "null handle");
+  int rc = drain_events(L);
+  if (rc) return rc;
+  L->options = options;
+  for (int k = 0; k < KC_COUNT; ++k) { L->ms[k] = 0.0; L->cnt[k] = 0; }
+  return NH_OK;
+}
+
+int nh_kernel_time(nh_lattice* L, int which, double* ms_total, long* launches) {
+  if (!L || which < 0 || which >= KC_COUNT) return fail(NH_EINVAL, "bad arguments");
+  int rc = drain_events(L);
+  if (rc) return rc;
+  if (ms_total) *ms_total = L->ms[which];
+  if (launches) *launches = L->cnt[which];
+  return NH_OK;
+}
+
+void nh_free(nh_lattice* L) {
+  if (!L) return;
+  for (auto& pr : L->pool) { cudaEventDestroy(pr.a); cudaEventDestroy(pr.b); }
+  delete L;
+}
+
+}  // extern "C"

@@ -1,0 +1,218 @@
+// nh_fd.cuh -- finite-difference kernels of the director side, baseline ("direct") variant:
+// one thread per fluid cell, neighbours read straight from global memory through L1.
+// nh_fd_tile.cuh holds the shared-memory tiled variant that the library uses by default; this
+// one stays as the simple form the tiled one is checked against (option NH_OPT_FD_DIRECT).
+//
+// PAPER.md:101-112 (Sec. II.B): central differences Eq. 13, solid node values fixed, director
+// equation Eq. 9 with D, W of Eq. 5, predictor-corrector;
+// molecular field Eq. 10 for the one-constant energy with chiral term (
+// DESIGN.md readings G1, G2); elastic stress Eq. 6 and force Eq. 12.
+#pragma once
+#include <cuda_runtime.h>
+#include "nh_lb.cuh"
+
+namespace nh {
+
+template <typename T>
+struct FdConst {
+  T K;          // Frank modulus
+  T Kq0;        // K * q0
+  T inv_gamma1; // 1/gamma1
+  T xi;         // flow alignment
+  T dt;         // Delta t_FD = r
+};
+
+template <typename T> struct V3 { T x, y, z; };
+
+template <typename T>
+__device__ __forceinline__ V3<T> ld3(const T* __restrict__ a, size_t N, unsigned c) {
+  V3<T> v; v.x = __ldg(a + c); v.y = __ldg(a + N + c); v.z = __ldg(a + 2 * N + c); return v;
+}
+template <typename T> __device__ __forceinline__ V3<T> operator-(V3<T> a, V3<T> b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+template <typename T> __device__ __forceinline__ V3<T> operator+(V3<T> a, V3<T> b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+template <typename T> __device__ __forceinline__ V3<T> operator*(T s, V3<T> a) { return {s * a.x, s * a.y, s * a.z}; }
+template <typename T> __device__ __forceinline__ T dot(V3<T> a, V3<T> b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+template <typename T> __device__ __forceinline__ V3<T> cross(V3<T> a, V3<T> b) {
+  return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
+}
+__device__ __forceinline__ float rsq(float s) { return 1.0f / sqrtf(s); }
+__device__ __forceinline__ double rsq(double s) { return 1.0 / sqrt(s); }
+template <typename T> __device__ __forceinline__ V3<T> unit(V3<T> v) { return rsq(dot(v, v)) * v; }
+
+// Six neighbours of a cell (periodic x, y; z neighbours always exist for a fluid cell).
+struct Nbr { unsigned xm, xp, ym, yp, zm, zp, c; };
+__device__ __forceinline__ Nbr neighbours(const Geom& G, int x, int y, int z) {
+  const int nx = G.nx;
+  const unsigned row = (unsigned)z * G.plane + (unsigned)y * nx;
+  const unsigned rz = (unsigned)z * G.plane;
+  Nbr b;
+  b.c = row + x;
+  b.xm = row + (x == 0 ? nx - 1 : x - 1);
+  b.xp = row + (x == nx - 1 ? 0 : x + 1);
+  b.ym = rz + (unsigned)(y == 0 ? G.ny - 1 : y - 1) * nx + x;
+  b.yp = rz + (unsigned)(y == G.ny - 1 ? 0 : y + 1) * nx + x;
+  b.zm = b.c - G.plane;
+  b.zp = b.c + G.plane;
+  return b;
+}
+
+// Right-hand side of Eq. 9 at one cell from the centre value and the six neighbours of m and u.
+//   h   = K lap m - 2 K q0 curl m          (7-point Laplacian, central curl)
+//   R   = h/gamma1 + xi m.D - (u.grad) m + W.m,   D, W as printed in Eq. 5
+//   R  <- R - (m.R) m                      (reading G3)
+// d?m = central difference of m along ?, s?m = m(+) + m(-) along ?; same for u.
+template <typename T>
+__device__ __forceinline__ V3<T> director_rhs(const FdConst<T>& C, V3<T> m, V3<T> mxm, V3<T> mxp,
+                                              V3<T> mym, V3<T> myp, V3<T> mzm, V3<T> mzp, V3<T> u,
+                                              V3<T> dxu, V3<T> dyu, V3<T> dzu) {
+  const T h = T(0.5);
+  const V3<T> dxm = h * (mxp - mxm), dym = h * (myp - mym), dzm = h * (mzp - mzm);
+  const V3<T> lap = ((mxp + mxm) + (myp + mym)) + (mzp + mzm) - T(6) * m;
+  const V3<T> curl = {dym.z - dzm.y, dzm.x - dxm.z, dxm.y - dym.x};
+  V3<T> R = C.inv_gamma1 * (C.K * lap - (T(2) * C.Kq0) * curl);
+  // velocity gradient G[b][c] = d_b u_c: rows dxu, dyu, dzu
+  // (m.D)_mu = m_a D_{a mu} = 1/2 m_a (d_a u_mu + d_mu u_a)
+  // (W.m)_mu = W_{mu a} m_a = 1/2 (d_a u_mu - d_mu u_a) m_a
+  // so  xi m.D + W.m = (xi+1)/2 (m.grad) u + (xi-1)/2 grad(u).m
+  const V3<T> mgu = m.x * dxu + (m.y * dyu + m.z * dzu);            // m_a d_a u_mu
+  const V3<T> gum = {dot(dxu, m), dot(dyu, m), dot(dzu, m)};       // d_mu u_a m_a
+  const V3<T> adv = u.x * dxm + (u.y * dym + u.z * dzm);            // u_a d_a m_mu
+  R = R + (h * (C.xi + T(1))) * mgu + (h * (C.xi - T(1))) * gum - adv;
+  return R - dot(m, R) * m;
+}
+
+// RHS at cell (x, y, z) of field m with velocity u, everything from global memory.
+template <typename T>
+__device__ __forceinline__ V3<T> rhs_global(const FdConst<T>& C, const T* __restrict__ m,
+                                            const T* __restrict__ u, size_t N, const Nbr& b,
+                                            bool with_flow) {
+  const V3<T> mc = ld3(m, N, b.c);
+  V3<T> uc = {T(0), T(0), T(0)}, dxu = uc, dyu = uc, dzu = uc;
+  if (with_flow) {
+    uc = ld3(u, N, b.c);
+    dxu = T(0.5) * (ld3(u, N, b.xp) - ld3(u, N, b.xm));
+    dyu = T(0.5) * (ld3(u, N, b.yp) - ld3(u, N, b.ym));
+    dzu = T(0.5) * (ld3(u, N, b.zp) - ld3(u, N, b.zm));
+  }
+  return director_rhs(C, mc, ld3(m, N, b.xm), ld3(m, N, b.xp), ld3(m, N, b.ym), ld3(m, N, b.yp),
+                      ld3(m, N, b.zm), ld3(m, N, b.zp), uc, dxu, dyu, dzu);
+}
+
+// Predictor: n^P = normalise(n + dt R[n]) on fluid cells.
+template <typename T>
+__global__ void __launch_bounds__(256)
+predictor_direct_kernel(const T* __restrict__ n, const T* __restrict__ u, T* __restrict__ nP,
+                        Geom G, FdConst<T> C, int with_flow) {
+  const unsigned k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= G.nfluid) return;
+  int x, y, z;
+  cell_of(k, G, x, y, z);
+  const Nbr b = neighbours(G, x, y, z);
+  const V3<T> k1 = rhs_global(C, n, u, G.N, b, with_flow != 0);
+  const V3<T> v = unit(ld3(n, G.N, b.c) + C.dt * k1);
+  nP[b.c] = v.x; nP[G.N + b.c] = v.y; nP[2 * G.N + b.c] = v.z;
+}
+
+// Corrector: n' = normalise(n + dt/2 (R[n] + R[n^P])), same u.
+template <typename T>
+__global__ void __launch_bounds__(256)
+corrector_direct_kernel(const T* __restrict__ n, const T* __restrict__ nP, const T* __restrict__ u,
+                        T* __restrict__ nnew, Geom G, FdConst<T> C, int with_flow) {
+  const unsigned k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= G.nfluid) return;
+  int x, y, z;
+  cell_of(k, G, x, y, z);
+  const Nbr b = neighbours(G, x, y, z);
+  const V3<T> k1 = rhs_global(C, n, u, G.N, b, with_flow != 0);
+  const V3<T> k2 = rhs_global(C, nP, u, G.N, b, with_flow != 0);
+  const V3<T> v = unit(ld3(n, G.N, b.c) + (T(0.5) * C.dt) * (k1 + k2));
+  nnew[b.c] = v.x; nnew[G.N + b.c] = v.y; nnew[2 * G.N + b.c] = v.z;
+}
+
+// Column b of the elastic stress at one cell: s_a = sigma_{a b},
+//   sigma_ab = -K d_a n . d_b n  +  K q0 (n x d_a n)_b          (Eq. 6; the chiral part is
+//   -K q0 eps_{mu b c} n_mu d_a n_c written as a cross product)
+template <typename T>
+__device__ __forceinline__ V3<T> stress_column(const FdConst<T>& C, int b, V3<T> n, V3<T> dxn,
+                                               V3<T> dyn, V3<T> dzn) {
+  const V3<T> db = (b == 0) ? dxn : (b == 1 ? dyn : dzn);
+  const V3<T> cx = cross(n, dxn), cy = cross(n, dyn), cz = cross(n, dzn);
+  const T qx = (b == 0) ? cx.x : (b == 1 ? cx.y : cx.z);
+  const T qy = (b == 0) ? cy.x : (b == 1 ? cy.y : cy.z);
+  const T qz = (b == 0) ? cz.x : (b == 1 ? cz.y : cz.z);
+  return {C.Kq0 * qx - C.K * dot(dxn, db), C.Kq0 * qy - C.K * dot(dyn, db), C.Kq0 * qz - C.K * dot(dzn, db)};
+}
+
+// sigma_{. b} at the cell (x, y, z) read from global memory; zero on the plate layers (reading G6).
+template <typename T>
+__device__ __forceinline__ V3<T> stress_column_at(const FdConst<T>& C, int b, const T* __restrict__ n,
+                                                  const Geom& G, int x, int y, int z) {
+  if (z == 0 || z == G.nz - 1) return {T(0), T(0), T(0)};
+  const Nbr q = neighbours(G, x, y, z);
+  const T h = T(0.5);
+  return stress_column(C, b, ld3(n, G.N, q.c), h * (ld3(n, G.N, q.xp) - ld3(n, G.N, q.xm)),
+                       h * (ld3(n, G.N, q.yp) - ld3(n, G.N, q.ym)), h * (ld3(n, G.N, q.zp) - ld3(n, G.N, q.zm)));
+}
+
+// Force (Eq. 12, last term): F_a = sum_b [sigma_ab(x + e_b) - sigma_ab(x - e_b)]/2.
+template <typename T>
+__global__ void __launch_bounds__(256)
+force_direct_kernel(const T* __restrict__ n, T* __restrict__ F, Geom G, FdConst<T> C) {
+  const unsigned k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= G.nfluid) return;
+  int x, y, z;
+  cell_of(k, G, x, y, z);
+  const int xm = (x == 0) ? G.nx - 1 : x - 1, xp = (x == G.nx - 1) ? 0 : x + 1;
+  const int ym = (y == 0) ? G.ny - 1 : y - 1, yp = (y == G.ny - 1) ? 0 : y + 1;
+  V3<T> f = stress_column_at(C, 0, n, G, xp, y, z) - stress_column_at(C, 0, n, G, xm, y, z);
+  f = f + (stress_column_at(C, 1, n, G, x, yp, z) - stress_column_at(C, 1, n, G, x, ym, z));
+  f = f + (stress_column_at(C, 2, n, G, x, y, z + 1) - stress_column_at(C, 2, n, G, x, y, z - 1));
+  const size_t c = (size_t)k + G.plane;
+  F[c] = T(0.5) * f.x; F[G.N + c] = T(0.5) * f.y; F[2 * G.N + c] = T(0.5) * f.z;
+}
+
+// ---- set_director helpers ---------------------------------------------------------------------
+// flag |= 1 if any input vector has zero or non-finite length
+__global__ void __launch_bounds__(256)
+check_director_kernel(const double* __restrict__ in, size_t N, int* __restrict__ flag) {
+  const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= N) return;
+  const double a = in[c], b = in[N + c], d = in[2 * N + c];
+  const double len = sqrt(a * a + b * b + d * d);
+  if (!(len > 0.0) || !isfinite(len)) atomicOr(flag, 1);
+}
+
+// normalise in FP64, overwrite the plates with z_hat, store in the device precision
+// into n, n^P and the corrector's output buffer (so its plates are set too)
+template <typename T>
+__global__ void __launch_bounds__(256)
+store_director_kernel(const double* __restrict__ in, T* __restrict__ n, T* __restrict__ nP,
+                      T* __restrict__ nnew, Geom G) {
+  const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= G.N) return;
+  const unsigned zz = (unsigned)(c / G.plane);
+  double a = 0.0, b = 0.0, d = 1.0;
+  if (zz != 0 && zz != (unsigned)G.nz - 1) {
+    a = in[c]; b = in[G.N + c]; d = in[2 * G.N + c];
+    const double len = sqrt(a * a + b * b + d * d);
+    a /= len; b /= len; d /= len;
+  }
+  n[c] = (T)a; n[G.N + c] = (T)b; n[2 * G.N + c] = (T)d;
+  nP[c] = (T)a; nP[G.N + c] = (T)b; nP[2 * G.N + c] = (T)d;
+  nnew[c] = (T)a; nnew[G.N + c] = (T)b; nnew[2 * G.N + c] = (T)d;
+}
+
+__global__ void __launch_bounds__(256) fill_f64_kernel(double* __restrict__ p, double v, size_t n) {
+  const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c < n) p[c] = v;
+}
+
+// device precision -> FP64 staging for nh_get_fields (whole grid, 3 components)
+template <typename T>
+__global__ void __launch_bounds__(256)
+widen3_kernel(const T* __restrict__ a, double* __restrict__ out, size_t n3) {
+  const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c < n3) out[c] = (double)a[c];
+}
+
+}  // namespace nh

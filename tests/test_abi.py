@@ -1,0 +1,96 @@
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/nh.h declares,
+validates its arguments, and refuses to compute without a CUDA device (no CPU fallback)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+import paper_2503_06610_b200 as nh
+from paper_2503_06610_b200 import build as nh_build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    nh_build.build()
+    return nh.load()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "nh.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(nh_[a-z_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = declared_symbols()
+    assert set(names) == set(nh.binding.EXPORTS)
+    for name in names:
+        assert hasattr(lib, name), name
+
+
+def test_workspace_bytes_and_validation(lib):
+    p = nh.make_params(16, 16, 8, 0.8, precision=nh.FP32_SHIFTED)
+    N = 16 * 16 * 8
+    b32 = nh.workspace_bytes(p)
+    assert b32 >= (2 * 19 + 5 * 3) * N * 4 + 3 * N * 8
+    assert b32 <= (2 * 19 + 5 * 3) * N * 4 + 3 * N * 8 + 9 * 256
+    p64 = nh.make_params(16, 16, 8, 0.8, precision=nh.FP64_SHIFTED)
+    assert nh.workspace_bytes(p64) >= (2 * 19 + 5 * 3) * N * 8 + 3 * N * 8
+    for bad in (dict(tau=0.5), dict(nz=2), dict(gamma1=0.0), dict(K=-1.0), dict(fd_ratio=-1),
+                dict(W0=0.1), dict(precision=7), dict(anchoring=1), dict(nx=0), dict(coupling=4),
+                dict(nx=4096, ny=4096, nz=64)):
+        kw = dict(nx=4, ny=4, nz=5, tau=0.8)
+        kw.update(bad)
+        q = nh.make_params(**kw)
+        assert nh.workspace_bytes(q) == 0
+        h = C.c_void_p()
+        rc = lib.nh_init_lattice(C.byref(q), 256, 1 << 20, None, C.byref(h))
+        assert rc == -1 and not h.value
+        assert lib.nh_last_error()
+    assert nh.workspace_bytes(nh.make_params(512, 512, 128, 0.8)) < 8 * 2 ** 30  # BASELINE: "roughly 7 GB"
+
+
+def test_null_and_small_workspace(lib):
+    p = nh.make_params(4, 4, 5, 0.8)
+    h = C.c_void_p()
+    assert lib.nh_init_lattice(C.byref(p), None, 1 << 20, None, C.byref(h)) == -1
+    assert lib.nh_init_lattice(C.byref(p), 256, 16, None, C.byref(h)) == -2
+    assert lib.nh_init_lattice(C.byref(p), 257, 1 << 20, None, C.byref(h)) == -1
+    assert lib.nh_step(None, 1, 1) == -1
+    assert lib.nh_set_director(None, None) == -1
+    assert lib.nh_get_fields(None, None, None, None, None) == -1
+    assert lib.nh_time(None) == -1
+    lib.nh_free(None)
+
+
+def test_no_cpu_fallback(lib):
+    """Without a CUDA device the library must fail loudly, not compute on the host."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    p = nh.make_params(4, 4, 5, 0.8)
+    h = C.c_void_p()
+    rc = lib.nh_init_lattice(C.byref(p), 256, 1 << 20, None, C.byref(h))
+    assert rc == -3 and not h.value
+    assert b"no CUDA device" in lib.nh_last_error()
+    with pytest.raises(RuntimeError):
+        nh.Lattice(4, 4, 5, 0.8)
+
+
+def test_product_does_not_import_the_oracle():
+    """The oracle is test infrastructure: nothing under the package or include/ may reference it."""
+    pkg = os.path.join(ROOT, "paper_2503_06610_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, fn)).read()
+                assert "import oracle" not in src and "from oracle" not in src, fn
+                assert "nh_oracle" not in src, fn
+    for fn in os.listdir(os.path.join(ROOT, "oracle")):
+        if fn.endswith((".py", ".cpp", ".h")):
+            src = open(os.path.join(ROOT, "oracle", fn)).read()
+            assert "paper_2503_06610_b200 import" not in src and "import paper_2503_06610_b200" not in src, fn
+            assert "nh_lb.cuh" not in src and "include/nh.h" not in src, fn

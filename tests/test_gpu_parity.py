@@ -1,0 +1,213 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances are BASELINE.json's: FP64 relative L_inf <= 1e-10 on u and n after 100 steps; shifted
+FP32 max|du|/max|u| <= 1e-3 and max|dn| <= 1e-4 after 1000 steps; the unshifted FP32 error is
+reported (printed), not gated.
+"""
+import numpy as np
+import pytest
+
+import nh_inputs as I
+from oracle import Oracle
+
+pytestmark = pytest.mark.gpu
+
+FP64_TOL = 1e-10
+FP32_TOL_U = 1e-3
+FP32_TOL_N = 1e-4
+
+
+def nh():
+    import paper_2503_06610_b200 as m
+    from paper_2503_06610_b200 import build
+    build.build()
+    return m
+
+
+def pair(p, precision, options=0):
+    """(oracle, gpu lattice) for a config dict from nh_inputs.config()."""
+    p = dict(p)
+    d = p.pop("director")
+    p.pop("steps", None)
+    o = Oracle(**dict(p, precision=precision))
+    o.set_director(d)
+    g = nh().Lattice(**dict(p, precision=precision))
+    if options:
+        g.set_options(options)
+    g.set_director(d)
+    return o, g
+
+
+def rel_linf(a, b):
+    return np.abs(a - b).max() / max(np.abs(b).max(), 1e-300)
+
+
+def compare(o, g, tol_u, tol_n, tol_f=None, label=""):
+    fo, fg = o.get_fields(), g.get_fields()
+    eu = rel_linf(fg["u"], fo["u"])
+    en = np.abs(fg["n"] - fo["n"]).max()
+    er = np.abs(fg["rho"] - fo["rho"]).max()
+    ef = rel_linf(fg["F"], fo["F"]) if np.abs(fo["F"]).max() > 0 else np.abs(fg["F"]).max()
+    print("%s t=%d  rel|du|=%.3e  max|dn|=%.3e  max|drho|=%.3e  rel|dF|=%.3e" % (label, o.time, eu, en, er, ef))
+    assert g.time == o.time
+    assert eu <= tol_u, (label, eu)
+    assert en <= tol_n, (label, en)
+    assert ef <= (tol_f if tol_f is not None else 100 * tol_u), (label, ef)
+    return eu, en
+
+
+@pytest.mark.parametrize("precision", [0, 3])
+def test_config0_fp64(precision):
+    """configs[0]: 16x16x8 noisy homeotropic channel, 200 steps, r = 1, FP64."""
+    o, g = pair(I.config(0), precision)
+    compare(o, g, 1e-300 + FP64_TOL, FP64_TOL, label="init")
+    for _ in range(2):
+        o.step(100)
+        g.step(100)
+        compare(o, g, FP64_TOL, FP64_TOL, label="cfg0 fp64 p%d" % precision)
+    f = g.get_fields()
+    for zz in (0, -1):  # plates: rho = 1, u = 0, F = 0, n = z_hat
+        assert np.all(f["rho"][zz] == 1.0) and np.all(f["u"][:, zz] == 0.0) and np.all(f["F"][:, zz] == 0.0)
+        assert np.all(f["n"][2, zz] == 1.0) and np.all(f["n"][:2, zz] == 0.0)
+
+
+def test_config0_fp32_shifted_and_unshifted():
+    """configs[0] in FP32: shifted within tolerance at 200 and 1000 steps; unshifted reported."""
+    o, g = pair(I.config(0), 1)
+    _, gu = pair(I.config(0), 2)
+    for n in (200, 800):
+        o.step(n)
+        g.step(n)
+        gu.step(n)
+        compare(o, g, FP32_TOL_U, FP32_TOL_N, tol_f=2e-3, label="cfg0 fp32 shifted")
+        fo, fu = o.get_fields(), gu.get_fields()
+        print("cfg0 fp32 UNSHIFTED t=%d rel|du|=%.3e max|dn|=%.3e (reported, not gated)"
+              % (o.time, rel_linf(fu["u"], fo["u"]), np.abs(fu["n"] - fo["n"]).max()))
+
+
+@pytest.mark.parametrize("precision,tol_u,tol_n", [(0, FP64_TOL, FP64_TOL), (1, FP32_TOL_U, FP32_TOL_N)])
+def test_config1_skyrmion_tube(precision, tol_u, tol_n):
+    """configs[1]: 64x64x32 single skyrmion tube in Poiseuille flow, chiral (p = 16), r = 1."""
+    o, g = pair(I.config(1), precision)
+    compare(o, g, 1e-300 + tol_u, tol_n, label="init")
+    o.step(100)
+    g.step(100)
+    compare(o, g, tol_u, tol_n, label="cfg1 p%d" % precision)
+
+
+@pytest.mark.parametrize("r", [2, 5, 10])
+@pytest.mark.parametrize("precision", [0, 1])
+def test_fd_ratio_schedule(r, precision):
+    """Sub-cycling: FD fires every r steps with Delta t_FD = r; step() called in
+    uneven chunks must give the same result as the oracle's single call."""
+    p = I.config(0, fd_ratio=r)
+    o, g = pair(p, precision)
+    o.step(60)
+    for chunk in (1, 7, r, 60 - 8 - r):
+        g.step(chunk)
+    tol = (FP64_TOL, FP64_TOL) if precision == 0 else (FP32_TOL_U, FP32_TOL_N)
+    compare(o, g, *tol, label="r=%d p%d" % (r, precision))
+    # explicit n_fd overrides the default, 0 freezes the director
+    n_before = g.get_fields(which=("n",))["n"].copy()
+    o.step(9, 0)
+    g.step(9, 0)
+    assert np.array_equal(g.get_fields(which=("n",))["n"], n_before)
+    o.step(6, 3)
+    g.step(6, 3)
+    compare(o, g, *tol, label="r=3 override p%d" % precision)
+
+
+@pytest.mark.parametrize("shape", [(17, 5, 6), (1, 1, 3), (3, 2, 9), (130, 3, 4), (33, 31, 5)])
+def test_ragged_and_degenerate_grids(shape):
+    """Sizes that are not multiples of the block / tile / vector width, down to a single fluid cell."""
+    nx, ny, nz = shape
+    d = I.noisy_homeotropic(nx, ny, nz, 0.1)
+    p = dict(nx=nx, ny=ny, nz=nz, tau=0.7, K=0.015, pitch=9.0, xi=0.8, gamma1=1.3,
+             g=(2e-6, -1e-6, 0.0), fd_ratio=2, director=d)
+    for precision, tol in ((0, (FP64_TOL, FP64_TOL)), (1, (FP32_TOL_U, FP32_TOL_N))):
+        o, g = pair(p, precision)
+        o.step(40)
+        g.step(40)
+        compare(o, g, *tol, tol_f=None if precision == 0 else 5e-3, label="ragged %s p%d" % (shape, precision))
+
+
+@pytest.mark.parametrize("coupling", [0, 1, 2])
+def test_coupling_switches(coupling):
+    p = I.config(0, coupling=coupling, fd_ratio=2)
+    o, g = pair(p, 0)
+    o.step(50)
+    g.step(50)
+    compare(o, g, FP64_TOL, FP64_TOL, label="coupling=%d" % coupling)
+
+
+def test_poiseuille_closed_form_on_gpu():
+    """The GPU itself reproduces the exact discrete Poiseuille profile (pin P1) in FP64."""
+    nz, tau, gx = 8, 0.8, 1e-6
+    nu = (tau - 0.5) / 3.0
+    g = nh().Lattice(4, 3, nz, tau, g=(gx, 0, 0), fd_ratio=0, precision=0, coupling=0)
+    g.step(4000, 0)
+    ux = g.get_fields(which=("u",))["u"][0]
+    z = np.arange(nz, dtype=np.float64)
+    exact = gx / (2 * nu) * (z - 0.5) * (nz - 1.5 - z) + gx * (16 * (tau - 0.5) ** 2 - 3) / (24 * nu)
+    assert np.abs(ux[1:-1] - exact[1:-1, None, None]).max() / exact.max() < 1e-10
+
+
+def test_invariants_long_run_fp32():
+    """Properties that hold at any size: mass conserved, |n| = 1, plates fixed (FP32 shifted)."""
+    p = I.config(1, fd_ratio=5)
+    d = p.pop("director")
+    p.pop("steps")
+    g = nh().Lattice(**dict(p, precision=1))
+    g.set_director(d)
+    nf = p["nx"] * p["ny"] * (p["nz"] - 2)
+    g.step(2000)
+    f = g.get_fields()
+    assert abs((f["rho"][1:-1] - 1.0).sum()) / nf < 1e-7
+    assert np.abs(np.sqrt((f["n"] ** 2).sum(0)) - 1.0).max() < 5e-7
+    assert np.isfinite(f["u"]).all() and np.abs(f["u"]).max() < 0.01
+
+
+def test_set_director_rejects_bad_input_and_keeps_state():
+    m = nh()
+    g = m.Lattice(8, 8, 6, 0.8, K=0.01, precision=0)
+    d = I.noisy_homeotropic(8, 8, 6, 0.05)
+    g.set_director(d)
+    before = g.get_fields()
+    bad = d.copy()
+    bad[:, 2, 3, 4] = 0.0
+    with pytest.raises(m.NhError) as ei:
+        g.set_director(bad)
+    assert ei.value.code == -1
+    bad[0, 2, 3, 4] = np.nan
+    with pytest.raises(m.NhError):
+        g.set_director(bad)
+    after = g.get_fields()
+    for k in before:
+        assert np.array_equal(before[k], after[k])
+    with pytest.raises(m.NhError):
+        g.step(-1)
+
+
+def test_options_do_not_change_results():
+    """Scheduling / kernel-variant switches are bit-neutral or within round-off of each other."""
+    m = nh()
+    ref = None
+    for opt in (0, m.OPT_TIMING, m.OPT_GRAPH, m.OPT_FD_DIRECT, m.OPT_LB_SCALAR, m.OPT_FD_DIRECT | m.OPT_LB_SCALAR):
+        p = I.config(0, fd_ratio=3)
+        d = p.pop("director")
+        p.pop("steps")
+        g = m.Lattice(**dict(p, precision=0))
+        g.set_options(opt)
+        g.set_director(d)
+        g.step(50)
+        g.step(31)
+        f = g.get_fields()
+        if ref is None:
+            ref = f
+        else:
+            assert rel_linf(f["u"], ref["u"]) < 1e-12 and np.abs(f["n"] - ref["n"]).max() < 1e-13, opt
+        if opt & m.OPT_TIMING:
+            ms, cnt = g.kernel_time("lb")
+            assert cnt == 81 and ms > 0.0
+            assert g.kernel_time("predictor")[1] == 27
+        assert g.launch_count > 81
