@@ -71,14 +71,19 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic(precision):
-    """DRAM bytes per LB launch from the committed ncu --set full capture, or None."""
-    path = os.path.join(ROOT, "profiles", "lb_traffic.json")
+def ncu_traffic(precision_name, grid):
+    """DRAM bytes per LB launch from the committed ncu --set full capture (profiles/lb_traffic.csv), or None."""
+    path = os.path.join(ROOT, "profiles", "lb_traffic.csv")
     if not os.path.exists(path):
         return None
     try:
-        rec = json.load(open(path))
-        return rec.get(str(precision), {}).get("dram_bytes_per_launch")
+        want = "%dx%dx%d" % tuple(grid)
+        val = None
+        for line in open(path).read().splitlines()[1:]:
+            c = line.split(",")
+            if len(c) >= 4 and c[0] == precision_name and c[1] == want:
+                val = float(c[3])     # the last matching row is the newest capture
+        return val
     except Exception:
         return None
 
@@ -261,7 +266,7 @@ def main():
     alg_bytes = 41 * word * nf          # 19 read + 19 write + 3 (F^LC) words per fluid cell
     achieved = alg_bytes / (lb_avg * 1e-3) / 1e9 if lb_avg > 0 else 0.0
     roofline = {"bound": "hbm", "kernel": "lb_step (collide+stream+force)", "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(prec),
+                "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(args.precision, desc["grid"]),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
                 "avg_launch_ms": lb_avg, "launches_timed": lb_n, "share_of_step": lb_ms / total_k if total_k else None,
                 "kernel_ms": {k: round(v[0], 4) for k, v in kt.items()},
