@@ -66,7 +66,7 @@ typedef struct {
 } nh_params;
 
 /* Bytes of device memory the lattice needs for these parameters (0 if they are invalid).
- * Layout: two population buffers [19][N], n, n^P, n', u, F^LC [3][N]
+ * Layout: two population buffers [19][N], n, n^P, n', a, u, F^LC [3][N]
  * in the device precision, one FP64 staging buffer [3][N], each 256-byte aligned. */
 size_t nh_workspace_bytes(const nh_params* p);
 
@@ -98,16 +98,22 @@ long nh_time(const nh_lattice* L);
 /* Number of kernels this lattice has launched so far (bench.py's gpu_launches). */
 long nh_launch_count(const nh_lattice* L);
 
-/* Options (results do not depend on them):
- *   bit0 NH_OPT_GRAPH     replay nh_step through CUDA graphs (launch-bound small grids)
- *   bit1 NH_OPT_TIMING    bracket every kernel launch with a CUDA-event pair on the lattice's stream
- *   bit2 NH_OPT_FD_DIRECT use the one-thread-per-cell FD kernels instead of the tiled ones
- *   bit3 NH_OPT_LB_SCALAR use the one-cell-per-thread LB kernel instead of the wide one
+/* Options (results agree within round-off whatever they are):
+ *   bit0 NH_OPT_GRAPH         replay nh_step through CUDA graphs (launch-bound small grids)
+ *   bit1 NH_OPT_TIMING        bracket every kernel launch with a CUDA-event pair on the lattice's
+ *                             stream (ignored while graphs are on)
+ *   bit2 NH_OPT_FD_DIRECT     use the one-thread-per-cell FD kernels instead of the tiled ones
+ *   bit3 NH_OPT_LB_WIDE       use the 16-byte-per-thread LB kernel (needs nx % 4 == 0 in FP32, % 2 in FP64)
+ *   bit4 NH_OPT_NO_SERPENTINE sweep the populations in the same direction on every launch
+ *   bit5 NH_OPT_FD_NOVEC      stage the FD tiles element by element even where 16-byte copies fit
+ *   bits 8-15                 planes per CTA of the tiled FD kernels (0 = chosen by the library)
  * Setting options resets the timing accumulators. */
-#define NH_OPT_GRAPH      1
-#define NH_OPT_TIMING     2
-#define NH_OPT_FD_DIRECT  4
-#define NH_OPT_LB_SCALAR  8
+#define NH_OPT_GRAPH          1
+#define NH_OPT_TIMING         2
+#define NH_OPT_FD_DIRECT      4
+#define NH_OPT_LB_WIDE        8
+#define NH_OPT_NO_SERPENTINE 16
+#define NH_OPT_FD_NOVEC      32
 int nh_set_options(nh_lattice* L, int options);
 
 /* Accumulated CUDA-event time (ms) and number of launches of one kernel class since the last

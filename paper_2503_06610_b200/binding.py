@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libnh_b200.so")
 
 FP64_SHIFTED, FP32_SHIFTED, FP32_UNSHIFTED, FP64_UNSHIFTED = 0, 1, 2, 3
-OPT_GRAPH, OPT_TIMING, OPT_FD_DIRECT, OPT_LB_SCALAR = 1, 2, 4, 8
+OPT_GRAPH, OPT_TIMING, OPT_FD_DIRECT, OPT_LB_WIDE, OPT_NO_SERPENTINE, OPT_FD_NOVEC = 1, 2, 4, 8, 16, 32
 KERNEL_CLASSES = ("lb", "velocity", "predictor", "corrector", "force", "other")
 
 EXPORTS = ("nh_workspace_bytes", "nh_init_lattice", "nh_set_director", "nh_step", "nh_get_fields",

@@ -14,7 +14,9 @@
 #include <vector>
 
 #include "nh_fd.cuh"
+#include "nh_fd_tile.cuh"
 #include "nh_lb.cuh"
+#include "nh_lb_vec.cuh"
 
 namespace {
 
@@ -72,10 +74,12 @@ struct nh_lattice {
   void* n[2];       // director ping-pong; n[ncur] is the current director
   int ncur;
   void* nP;
+  void* a;          // n + dt/2 k1, predictor -> corrector (tiled FD kernels)
   void* u;
   void* F;
   double* stage;    // FP64 staging [3][N]
   int* flag;
+  int sweep;        // direction of the next population sweep (alternates, see sweep_block)
   // per-class CUDA-event timing (option bit1)
   struct Pair { cudaEvent_t a, b; int cls; };
   std::vector<Pair> pool;
@@ -154,12 +158,28 @@ nh::FdConst<T> fd_const(const nh_lattice* L, int r) {
 }
 
 // ---- typed launchers ----------------------------------------------------------------------------
+// direction of this population sweep; the next one runs the other way (NH_OPT_NO_SERPENTINE: always up)
+int next_sweep(nh_lattice* L) {
+  if (L->options & NH_OPT_NO_SERPENTINE) return 0;
+  const int r = L->sweep;
+  L->sweep ^= 1;
+  return r;
+}
+
 template <typename T, bool SH>
 int launch_lb(nh_lattice* L) {
   Bracket br(L, KC_LB);
   if (br.rc) return br.rc;
-  nh::lb_step_kernel<T, SH><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
-      (const T*)L->f[L->cur], (T*)L->f[L->cur ^ 1], (const T*)L->F, L->G, lb_const<T>(L));
+  constexpr int V = 16 / (int)sizeof(T);
+  const int rev = next_sweep(L);
+  if ((L->options & NH_OPT_LB_WIDE) && L->G.nx % V == 0) {
+    const unsigned ngroups = L->G.nfluid / V;
+    nh::lb_step_vec_kernel<T, SH, V><<<blocks_for(ngroups), BLOCK, 0, L->stream>>>(
+        (const T*)L->f[L->cur], (T*)L->f[L->cur ^ 1], (const T*)L->F, L->G, lb_const<T>(L), ngroups, rev);
+  } else {
+    nh::lb_step_kernel<T, SH><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
+        (const T*)L->f[L->cur], (T*)L->f[L->cur ^ 1], (const T*)L->F, L->G, lb_const<T>(L), rev);
+  }
   br.end();
   return NH_OK;
 }
@@ -167,17 +187,58 @@ template <typename T, bool SH>
 int launch_velocity(nh_lattice* L) {
   Bracket br(L, KC_VEL);
   if (br.rc) return br.rc;
+  // reads what the LB launch just wrote, starting where that launch ended; the next LB launch
+  // then starts where this one ended
+  const int rev = next_sweep(L);
   nh::velocity_kernel<T, SH><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
-      (const T*)L->f[L->cur], (const T*)L->F, (T*)L->u, L->G, lb_const<T>(L));
+      (const T*)L->f[L->cur], (const T*)L->F, (T*)L->u, L->G, lb_const<T>(L), rev);
   br.end();
   return NH_OK;
 }
+
+// z-march geometry of the tiled FD kernels: enough CTAs to fill 148 SMs several times over, but
+// chunks long enough that the 2 (director) or 4 (force) extra planes per chunk stay cheap
+struct TileGrid { dim3 grid; int zchunk; };
+TileGrid tile_grid(const nh_lattice* L) {
+  const int tiles = ((L->G.nx + nh::TX - 1) / nh::TX) * ((L->G.ny + nh::TY - 1) / nh::TY);
+  const int nzf = L->G.nz - 2;
+  int zchunk = (L->options >> 8) & 0xff;                     // tuning override
+  if (zchunk == 0) {
+    int want = (6 * 148 + tiles - 1) / tiles;                // chunks wanted
+    int most = (nzf + 7) / 8;                                // chunks of >= 8 planes
+    if (want > most) want = most;
+    if (want < 1) want = 1;
+    zchunk = (nzf + want - 1) / want;
+  }
+  if (zchunk > nzf) zchunk = nzf;
+  TileGrid g;
+  g.zchunk = zchunk;
+  g.grid = dim3((L->G.nx + nh::TX - 1) / nh::TX, (L->G.ny + nh::TY - 1) / nh::TY, (nzf + zchunk - 1) / zchunk);
+  return g;
+}
+// 16-byte staging copies need whole 32-cell rows on 16-byte boundaries
+bool tiles_vec(const nh_lattice* L) { return L->G.nx % nh::TX == 0 && !(L->options & NH_OPT_FD_NOVEC); }
+bool tiles_fit(const nh_lattice* L) {
+  const TileGrid g = tile_grid(L);
+  return g.grid.y <= 65535u && g.grid.z <= 65535u;
+}
+
 template <typename T>
 int launch_force(nh_lattice* L) {
   Bracket br(L, KC_FORCE);
   if (br.rc) return br.rc;
-  nh::force_direct_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
-      (const T*)L->n[L->ncur], (T*)L->F, L->G, fd_const<T>(L, 1));
+  if (!(L->options & NH_OPT_FD_DIRECT) && tiles_fit(L)) {
+    const TileGrid g = tile_grid(L);
+    if (tiles_vec(L))
+      nh::force_tile_kernel<T, true><<<g.grid, nh::TILE_THREADS, nh::force_smem_bytes<T>(), L->stream>>>(
+          (const T*)L->n[L->ncur], (T*)L->F, L->G, fd_const<T>(L, 1), g.zchunk);
+    else
+      nh::force_tile_kernel<T, false><<<g.grid, nh::TILE_THREADS, nh::force_smem_bytes<T>(), L->stream>>>(
+          (const T*)L->n[L->ncur], (T*)L->F, L->G, fd_const<T>(L, 1), g.zchunk);
+  } else {
+    nh::force_direct_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
+        (const T*)L->n[L->ncur], (T*)L->F, L->G, fd_const<T>(L, 1));
+  }
   br.end();
   return NH_OK;
 }
@@ -185,21 +246,51 @@ template <typename T>
 int launch_director(nh_lattice* L, int r) {
   const int with_flow = (L->p.coupling & 2) ? 1 : 0;
   const nh::FdConst<T> C = fd_const<T>(L, r);
+  const bool tiled = !(L->options & NH_OPT_FD_DIRECT) && tiles_fit(L);
+  const TileGrid g = tile_grid(L);
   {
     Bracket br(L, KC_PRED);
     if (br.rc) return br.rc;
-    nh::predictor_direct_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
-        (const T*)L->n[L->ncur], (const T*)L->u, (T*)L->nP, L->G, C, with_flow);
+    if (tiled && tiles_vec(L))
+      nh::director_tile_kernel<T, 0, true><<<g.grid, nh::TILE_THREADS, nh::director_smem_bytes<T>(), L->stream>>>(
+          (const T*)L->n[L->ncur], (const T*)L->u, nullptr, (T*)L->nP, (T*)L->a, L->G, C, with_flow, g.zchunk);
+    else if (tiled)
+      nh::director_tile_kernel<T, 0, false><<<g.grid, nh::TILE_THREADS, nh::director_smem_bytes<T>(), L->stream>>>(
+          (const T*)L->n[L->ncur], (const T*)L->u, nullptr, (T*)L->nP, (T*)L->a, L->G, C, with_flow, g.zchunk);
+    else
+      nh::predictor_direct_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
+          (const T*)L->n[L->ncur], (const T*)L->u, (T*)L->nP, L->G, C, with_flow);
     br.end();
   }
   {
     Bracket br(L, KC_CORR);
     if (br.rc) return br.rc;
-    nh::corrector_direct_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
-        (const T*)L->n[L->ncur], (const T*)L->nP, (const T*)L->u, (T*)L->n[L->ncur ^ 1], L->G, C, with_flow);
+    if (tiled && tiles_vec(L))
+      nh::director_tile_kernel<T, 1, true><<<g.grid, nh::TILE_THREADS, nh::director_smem_bytes<T>(), L->stream>>>(
+          (const T*)L->nP, (const T*)L->u, (const T*)L->a, (T*)L->n[L->ncur ^ 1], nullptr, L->G, C, with_flow, g.zchunk);
+    else if (tiled)
+      nh::director_tile_kernel<T, 1, false><<<g.grid, nh::TILE_THREADS, nh::director_smem_bytes<T>(), L->stream>>>(
+          (const T*)L->nP, (const T*)L->u, (const T*)L->a, (T*)L->n[L->ncur ^ 1], nullptr, L->G, C, with_flow, g.zchunk);
+    else
+      nh::corrector_direct_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
+          (const T*)L->n[L->ncur], (const T*)L->nP, (const T*)L->u, (T*)L->n[L->ncur ^ 1], L->G, C, with_flow);
     br.end();
   }
   L->ncur ^= 1;
+  return NH_OK;
+}
+
+// opt in to the dynamic shared memory the tiled kernels ask for (once per process and type)
+template <typename T>
+int enable_tile_smem() {
+  const int db = (int)nh::director_smem_bytes<T>(), fb = (int)nh::force_smem_bytes<T>();
+  const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+  NH_CUDA(cudaFuncSetAttribute(nh::director_tile_kernel<T, 0, true>, attr, db));
+  NH_CUDA(cudaFuncSetAttribute(nh::director_tile_kernel<T, 1, true>, attr, db));
+  NH_CUDA(cudaFuncSetAttribute(nh::director_tile_kernel<T, 0, false>, attr, db));
+  NH_CUDA(cudaFuncSetAttribute(nh::director_tile_kernel<T, 1, false>, attr, db));
+  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, true>, attr, fb));
+  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false>, attr, fb));
   return NH_OK;
 }
 
@@ -223,6 +314,8 @@ int step_typed(nh_lattice* L, int n_lb, int r) {
 template <typename T, bool SH>
 int init_typed(nh_lattice* L) {
   const size_t N = L->G.N;
+  { const int rc = enable_tile_smem<T>(); if (rc) return rc; }
+  NH_CUDA(cudaMemsetAsync(L->a, 0, 3 * N * sizeof(T), L->stream));
   for (int b = 0; b < 2; ++b) {
     Bracket br(L, KC_OTHER);
     nh::rest_kernel<T, SH><<<blocks_for(N), BLOCK, 0, L->stream>>>((T*)L->f[b], L->G);
@@ -310,7 +403,7 @@ size_t nh_workspace_bytes(const nh_params* p) {
   const size_t w = word_of(p->precision);
   size_t b = 0;
   b += 2 * align_up(19 * N * w);   // populations A, B
-  b += 5 * align_up(3 * N * w);    // n[0], n[1], nP, u, F
+  b += 6 * align_up(3 * N * w);    // n[0], n[1], nP, a, u, F
   b += align_up(3 * N * sizeof(double));  // staging
   b += ALIGN;                      // flag
   return b;
@@ -339,14 +432,14 @@ int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_strea
   L->G.N = (size_t)L->G.plane * p->nz;
   L->q0 = p->pitch > 0.0 ? 2.0 * M_PI / p->pitch : 0.0;
   L->stream = (cudaStream_t)cuda_stream;
-  L->t = 0; L->launches = 0; L->options = 0; L->cur = 0; L->ncur = 0; L->used = 0;
+  L->t = 0; L->launches = 0; L->options = 0; L->cur = 0; L->ncur = 0; L->used = 0; L->sweep = 0;
   for (int k = 0; k < KC_COUNT; ++k) { L->ms[k] = 0.0; L->cnt[k] = 0; }
   const size_t N = L->G.N, w = word_of(p->precision);
   char* base = (char*)ws;
   auto take = [&](size_t b) { char* q = base; base += align_up(b); return (void*)q; };
   L->f[0] = take(19 * N * w); L->f[1] = take(19 * N * w);
   L->n[0] = take(3 * N * w); L->n[1] = take(3 * N * w);
-  L->nP = take(3 * N * w); L->u = take(3 * N * w); L->F = take(3 * N * w);
+  L->nP = take(3 * N * w); L->a = take(3 * N * w); L->u = take(3 * N * w); L->F = take(3 * N * w);
   L->stage = (double*)take(3 * N * sizeof(double));
   L->flag = (int*)take(sizeof(int));
   int rc;

@@ -159,12 +159,19 @@ __device__ __forceinline__ void cell_of(unsigned fluid_index, const Geom& G, int
   x = (int)(xy - yy * (unsigned)G.nx);
 }
 
+// Sweep direction.  Consecutive launches traverse the lattice in opposite directions: a launch
+// then starts on the cells whose populations the previous launch wrote last, which are still in
+// the 126 MB L2, so part of every gather is served without touching HBM.
+__device__ __forceinline__ unsigned sweep_block(int reverse) {
+  return reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
+}
+
 // One LB step, one thread per fluid cell (baseline variant; nh_lb_vec.cuh holds the wide one).
 template <typename T, bool SHIFTED>
 __global__ void __launch_bounds__(256)
 lb_step_kernel(const T* __restrict__ fsrc, T* __restrict__ fdst, const T* __restrict__ Flc,
-               Geom G, LbConst<T> C) {
-  const unsigned k = blockIdx.x * blockDim.x + threadIdx.x;
+               Geom G, LbConst<T> C, int reverse) {
+  const unsigned k = sweep_block(reverse) * blockDim.x + threadIdx.x;
   if (k >= G.nfluid) return;
   int x, y, z;
   cell_of(k, G, x, y, z);
@@ -183,8 +190,8 @@ lb_step_kernel(const T* __restrict__ fsrc, T* __restrict__ fdst, const T* __rest
 template <typename T, bool SHIFTED>
 __global__ void __launch_bounds__(256)
 velocity_kernel(const T* __restrict__ fsrc, const T* __restrict__ Flc, T* __restrict__ u,
-                Geom G, LbConst<T> C) {
-  const unsigned k = blockIdx.x * blockDim.x + threadIdx.x;
+                Geom G, LbConst<T> C, int reverse) {
+  const unsigned k = sweep_block(reverse) * blockDim.x + threadIdx.x;
   if (k >= G.nfluid) return;
   int x, y, z;
   cell_of(k, G, x, y, z);

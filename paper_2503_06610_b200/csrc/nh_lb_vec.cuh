@@ -187,8 +187,8 @@ __device__ __forceinline__ Where where_of(unsigned k, unsigned ngroups, const Ge
 template <typename T, bool SHIFTED, int V>
 __global__ void __launch_bounds__(256)
 lb_step_vec_kernel(const T* __restrict__ fsrc, T* __restrict__ fdst, const T* __restrict__ Flc,
-                   Geom G, LbConst<T> C, unsigned ngroups) {
-  const unsigned k = blockIdx.x * blockDim.x + threadIdx.x;
+                   Geom G, LbConst<T> C, unsigned ngroups, int reverse) {
+  const unsigned k = sweep_block(reverse) * blockDim.x + threadIdx.x;
   bool active;
   const Where w = where_of<V>(k, ngroups, G, active);
   PopV<T, V> P;

@@ -192,7 +192,7 @@ def test_options_do_not_change_results():
     """Scheduling / kernel-variant switches are bit-neutral or within round-off of each other."""
     m = nh()
     ref = None
-    for opt in (0, m.OPT_TIMING, m.OPT_GRAPH, m.OPT_FD_DIRECT, m.OPT_LB_SCALAR, m.OPT_FD_DIRECT | m.OPT_LB_SCALAR):
+    for opt in (0, m.OPT_TIMING, m.OPT_GRAPH, m.OPT_FD_DIRECT, m.OPT_LB_WIDE, m.OPT_FD_DIRECT | m.OPT_LB_WIDE):
         p = I.config(0, fd_ratio=3)
         d = p.pop("director")
         p.pop("steps")
