@@ -67,7 +67,8 @@ typedef struct {
 
 /* Bytes of device memory the lattice needs for these parameters (0 if they are invalid).
  * Layout: two population buffers [19][N], n, n^P, n', a, u, F^LC [3][N]
- * in the device precision, one FP64 staging buffer [3][N], each 256-byte aligned. */
+ * in the device precision, one FP64 staging buffer [3][N], the plane ring of the two-step LB
+ * kernel (min(nz-2, 12) planes of 19 populations) and its flags, each 256-byte aligned. */
 size_t nh_workspace_bytes(const nh_params* p);
 
 /* Create a lattice in `dev_workspace` (DEVICE pointer, 256-byte aligned, >= nh_workspace_bytes).
@@ -106,7 +107,11 @@ long nh_launch_count(const nh_lattice* L);
  *   bit3 NH_OPT_LB_WIDE       use the 16-byte-per-thread LB kernel (needs nx % 4 == 0 in FP32, % 2 in FP64)
  *   bit4 NH_OPT_NO_SERPENTINE sweep the populations in the same direction on every launch
  *   bit5 NH_OPT_FD_NOVEC      stage the FD tiles element by element even where 16-byte copies fit
+ *   bit6 NH_OPT_LB_TWOSTEP    two LB steps per launch through an L2-resident plane ring wherever no
+ *                             director update falls between them (bit-identical results)
  *   bits 8-15                 planes per CTA of the tiled FD kernels (0 = chosen by the library)
+ *   bits 16-19, 20-25         two-step kernel: lead D of phase 1 in planes, ring planes R (0 = default)
+ *   bits 26-29                two-step kernel: persistent CTAs per SM (0 = occupancy limit)
  * Setting options resets the timing accumulators. */
 #define NH_OPT_GRAPH          1
 #define NH_OPT_TIMING         2
@@ -114,12 +119,13 @@ long nh_launch_count(const nh_lattice* L);
 #define NH_OPT_LB_WIDE        8
 #define NH_OPT_NO_SERPENTINE 16
 #define NH_OPT_FD_NOVEC      32
+#define NH_OPT_LB_TWOSTEP    64
 int nh_set_options(nh_lattice* L, int options);
 
 /* Accumulated CUDA-event time (ms) and number of launches of one kernel class since the last
  * nh_set_options; synchronises the stream.  Time is only accumulated while NH_OPT_TIMING is set.
  * which: 0 = LB collide+stream, 1 = velocity (moments, u store), 2 = predictor, 3 = corrector,
- *        4 = force, 5 = everything else (conversions, initialisation). */
+ *        4 = force, 5 = everything else (conversions, initialisation), 6 = two-step LB launches. */
 int nh_kernel_time(nh_lattice* L, int which, double* ms_total, long* launches);
 
 void nh_free(nh_lattice* L);

@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 #include <string>
 #include <vector>
@@ -16,6 +17,7 @@
 #include "nh_fd.cuh"
 #include "nh_fd_tile.cuh"
 #include "nh_lb.cuh"
+#include "nh_lb2.cuh"
 #include "nh_lb_vec.cuh"
 
 namespace {
@@ -56,7 +58,15 @@ size_t word_of(int precision) {
   return (precision == NH_FP64_SHIFTED || precision == NH_FP64_UNSHIFTED) ? 8 : 4;
 }
 
-enum KernelClass { KC_LB = 0, KC_VEL = 1, KC_PRED = 2, KC_CORR = 3, KC_FORCE = 4, KC_OTHER = 5, KC_COUNT = 6 };
+enum KernelClass { KC_LB = 0, KC_VEL = 1, KC_PRED = 2, KC_CORR = 3, KC_FORCE = 4, KC_OTHER = 5, KC_LB2 = 6, KC_COUNT = 7 };
+
+// planes of the two-step kernel's ring (nh_lb2.cuh) that the workspace holds
+int ring_planes(const nh_params* p) { return p->nz - 2 < 12 ? p->nz - 2 : 12; }
+// u64 words of the two-step kernel's control block: 8 header words, then two u32 flags per plane and piece
+size_t wave_words(const nh_params* p) {
+  const size_t pieces = (size_t)p->nx * p->ny / 128 + p->ny + 1;   // upper bound over the piece shapes
+  return 8 + (size_t)(p->nz - 2) * pieces;
+}
 
 }  // namespace
 
@@ -80,6 +90,11 @@ struct nh_lattice {
   double* stage;    // FP64 staging [3][N]
   int* flag;
   int sweep;        // direction of the next population sweep (alternates, see sweep_block)
+  void* ring;       // plane ring of the two-step LB kernel
+  int ring_cap;     // planes it holds
+  unsigned long long* wave;   // device counters of the two-step kernel: err flag at [4], done1, done2 from [8]
+  unsigned long long wave_epoch, wave_tickets;
+  int sm_count, wave_ctas_per_sm;
   // per-class CUDA-event timing (option bit1)
   struct Pair { cudaEvent_t a, b; int cls; };
   std::vector<Pair> pool;
@@ -183,6 +198,85 @@ int launch_lb(nh_lattice* L) {
   br.end();
   return NH_OK;
 }
+// ---- two LB steps in one launch (nh_lb2.cuh) ----------------------------------------------------
+// Piece geometry for U cells per thread; false if this grid does not tile into pieces.
+struct PieceGrid { unsigned prows, ppr, rows_per_piece; int spr_shift; };
+int lb2_threads(const nh_lattice* L) { return (L->options >> 31) & 1 ? 128 : 256; }
+bool piece_grid(const nh_lattice* L, int U, PieceGrid* g) {
+  const unsigned nx = (unsigned)L->G.nx, ny = (unsigned)L->G.ny, seg = 32u * U, pc = (unsigned)lb2_threads(L) * U;
+  const unsigned warps = (unsigned)lb2_threads(L) / 32;
+  if (nx % seg) return false;
+  unsigned spr;
+  if (pc % nx == 0) { g->rows_per_piece = pc / nx; spr = nx / seg; g->prows = (ny + g->rows_per_piece - 1) / g->rows_per_piece; g->ppr = 1; }
+  else if (nx % pc == 0) { g->rows_per_piece = 1; spr = warps; g->prows = ny; g->ppr = nx / pc; }
+  else return false;
+  g->spr_shift = 0;
+  while ((1u << g->spr_shift) < spr) ++g->spr_shift;
+  return (1u << g->spr_shift) == spr;
+}
+int lb2_cells_per_thread(const nh_lattice* L) {
+  PieceGrid g;
+  int U = (L->options >> 30) & 1 ? 1 : 2;
+  for (; U >= 1; --U) if (piece_grid(L, U, &g)) return U;
+  return 0;
+}
+bool lb2_usable(const nh_lattice* L) {
+  return (L->options & NH_OPT_LB_TWOSTEP) && L->ring_cap >= 3 && lb2_cells_per_thread(L) > 0;
+}
+
+template <typename T, bool SH, int U, int NT>
+int launch_lb2_u(nh_lattice* L) {
+  Bracket br(L, KC_LB2);
+  if (br.rc) return br.rc;
+  const int nzf = L->G.nz - 2;
+  PieceGrid g;
+  piece_grid(L, U, &g);
+  nh::Wave W;
+  W.ticket = L->wave;
+  W.err = (int*)(L->wave + 4);
+  W.prows = g.prows; W.ppr = g.ppr; W.rows_per_piece = g.rows_per_piece; W.spr_shift = g.spr_shift;
+  W.cps = g.prows * g.ppr;
+  W.flag1 = (unsigned*)(L->wave + 8);
+  W.flag2 = W.flag1 + (size_t)nzf * W.cps;
+  W.nzf = nzf;
+  int D = (L->options >> 16) & 0xf, R = (L->options >> 20) & 0x3f;
+  if (D == 0) D = 4;
+  if (R == 0) R = D + 6;
+  if (R > L->ring_cap) R = L->ring_cap;
+  if (D > R - 2) D = R - 2;
+  W.D = D; W.R = R;
+  W.reverse = next_sweep(L);
+  { const char* e = getenv("NH_WAVE_DBG"); W.dbg = e ? atoi(e) : 0; }
+  const unsigned long long units = 2ull * nzf * W.cps;
+  int per_sm_max = 0;
+  NH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_max, nh::lb_wave_kernel<T, SH, U, NT>, NT, 0));
+  int per_sm = ((L->options >> 26) & 0xf);
+  if (per_sm == 0 || per_sm > per_sm_max) per_sm = per_sm_max;
+  if (per_sm < 1) return fail(NH_ECUDA, "two-step LB kernel does not fit on an SM");
+  unsigned long long grid = (unsigned long long)per_sm * L->sm_count;
+  if (grid > units) grid = units;
+  W.ticket_base = L->wave_tickets;
+  L->wave_tickets += units + 3 * grid;      // every CTA draws three tickets past the end
+  L->wave_epoch += 1;
+  W.epoch = (unsigned)L->wave_epoch;
+  nh::DirTab<const T> A;
+  nh::DirTab<T> Rg, B;
+  for (int i = 0; i < nh::Q; ++i) {
+    A.p[i] = (const T*)L->f[L->cur] + (size_t)i * L->G.N;
+    B.p[i] = (T*)L->f[L->cur ^ 1] + (size_t)i * L->G.N;
+    Rg.p[i] = (T*)L->ring + (size_t)i * R * L->G.plane;
+  }
+  nh::lb_wave_kernel<T, SH, U, NT><<<(unsigned)grid, NT, 0, L->stream>>>(A, Rg, B, (const T*)L->F, L->G, lb_const<T>(L), W);
+  br.end();
+  return NH_OK;
+}
+template <typename T, bool SH>
+int launch_lb2(nh_lattice* L) {
+  const bool two = lb2_cells_per_thread(L) == 2;
+  if (lb2_threads(L) == 128) return two ? launch_lb2_u<T, SH, 2, 128>(L) : launch_lb2_u<T, SH, 1, 128>(L);
+  return two ? launch_lb2_u<T, SH, 2, 256>(L) : launch_lb2_u<T, SH, 1, 256>(L);
+}
+
 template <typename T, bool SH>
 int launch_velocity(nh_lattice* L) {
   Bracket br(L, KC_VEL);
@@ -297,8 +391,17 @@ int enable_tile_smem() {
 template <typename T, bool SH>
 int step_typed(nh_lattice* L, int n_lb, int r) {
   for (int s = 0; s < n_lb; ++s) {
-    int rc = launch_lb<T, SH>(L);
-    if (rc) return rc;
+    int rc;
+    // two steps in one launch when no director update falls between them
+    if (s + 1 < n_lb && lb2_usable(L) && !(r > 0 && (L->t + 1) % r == 0)) {
+      rc = launch_lb2<T, SH>(L);
+      if (rc) return rc;
+      L->t += 1;
+      ++s;
+    } else {
+      rc = launch_lb<T, SH>(L);
+      if (rc) return rc;
+    }
     L->cur ^= 1;
     L->t += 1;
     if (r > 0 && L->t % r == 0) {
@@ -314,6 +417,11 @@ int step_typed(nh_lattice* L, int n_lb, int r) {
 template <typename T, bool SH>
 int init_typed(nh_lattice* L) {
   const size_t N = L->G.N;
+  {
+    int dev = 0;
+    NH_CUDA(cudaGetDevice(&dev));
+    NH_CUDA(cudaDeviceGetAttribute(&L->sm_count, cudaDevAttrMultiProcessorCount, dev));
+  }
   { const int rc = enable_tile_smem<T>(); if (rc) return rc; }
   NH_CUDA(cudaMemsetAsync(L->a, 0, 3 * N * sizeof(T), L->stream));
   for (int b = 0; b < 2; ++b) {
@@ -380,6 +488,11 @@ int get_fields_typed(nh_lattice* L, double* rho, double* u, double* n, double* F
   }
   NH_CUDA(cudaGetLastError());
   NH_CUDA(cudaStreamSynchronize(L->stream));
+  if (L->wave_epoch > 0) {   // a two-step launch whose wavefront stalled has produced garbage
+    int werr = 0;
+    NH_CUDA(cudaMemcpy(&werr, L->wave + 4, sizeof(int), cudaMemcpyDeviceToHost));
+    if (werr) return fail(NH_ECUDA, "two-step LB kernel: a wavefront dependency wait timed out");
+  }
   return NH_OK;
 }
 
@@ -406,6 +519,8 @@ size_t nh_workspace_bytes(const nh_params* p) {
   b += 6 * align_up(3 * N * w);    // n[0], n[1], nP, a, u, F
   b += align_up(3 * N * sizeof(double));  // staging
   b += ALIGN;                      // flag
+  b += align_up((size_t)ring_planes(p) * 19 * p->nx * p->ny * w);   // plane ring of the two-step LB kernel
+  b += align_up(wave_words(p) * 8);                                 // its counters
   return b;
 }
 
@@ -442,6 +557,12 @@ int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_strea
   L->nP = take(3 * N * w); L->a = take(3 * N * w); L->u = take(3 * N * w); L->F = take(3 * N * w);
   L->stage = (double*)take(3 * N * sizeof(double));
   L->flag = (int*)take(sizeof(int));
+  L->ring_cap = ring_planes(p);
+  L->ring = take((size_t)L->ring_cap * 19 * L->G.plane * w);
+  L->wave = (unsigned long long*)take(wave_words(p) * 8);
+  L->wave_epoch = 0; L->wave_tickets = 0;
+  e = cudaMemsetAsync(L->wave, 0, wave_words(p) * 8, L->stream);
+  if (e != cudaSuccess) { delete L; return cuda_fail(e, "cudaMemsetAsync(wave)"); }
   int rc;
   switch (p->precision) {
     case NH_FP64_SHIFTED: rc = init_typed<double, true>(L); break;

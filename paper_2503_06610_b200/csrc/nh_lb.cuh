@@ -41,51 +41,84 @@ struct LbConst {
 template <typename T>
 struct Pop { T f[Q]; };
 
-template <typename T>
-__device__ __forceinline__ T ldg_stream(const T* p) { return __ldg(p); }
+__device__ __forceinline__ float fmaf_t(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fmaf_t(double a, double b, double c) { return fma(a, b, c); }
 
-// Gather f_i(x, t) for the cell (x, y, z) from the post-collision buffer `fs`.
-template <typename T>
-__device__ __forceinline__ void pull(const T* __restrict__ fs, const Geom& G, int x, int y, int z,
-                                     Pop<T>& P) {
-  const size_t N = G.N;
+// Load policies of the gathers: LD_NC read-only path (data not written during the launch),
+// LD_CS the same with the streaming (evict-first) hint, LD_CG coherent at L2 (data that another CTA
+// of the SAME launch has written: the ring of the two-step kernel, nh_lb2.cuh).
+// LD_PF loads nothing: it asks the L2 to fetch the line (the two-step kernel warms the next unit).
+enum { LD_NC = 0, LD_CS = 1, LD_CG = 2, LD_PF = 3 };
+template <typename T, int LD>
+__device__ __forceinline__ T ldp(const T* p) {
+  if constexpr (LD == LD_NC) return __ldg(p);
+  else if constexpr (LD == LD_CS) return __ldcs(p);
+  else if constexpr (LD == LD_CG) return __ldcg(p);
+  else { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); return T(0); }
+}
+
+// Where the three z planes a gather touches live inside a population array: element offsets of
+// the planes z-1, z, z+1 and the stride between directions.  The lattice arrays use
+// (z-1, z, z+1)*plane and stride N; the plane ring of nh_lb2.cuh maps planes to ring slots.
+struct PlaneMap {
+  size_t stride;
+  unsigned zm, z0, zp;
+};
+__device__ __forceinline__ PlaneMap lattice_map(const Geom& G, int z) {
+  PlaneMap M;
+  M.stride = G.N;
+  M.z0 = (unsigned)z * G.plane;
+  M.zm = M.z0 - G.plane;
+  M.zp = M.z0 + G.plane;
+  return M;
+}
+
+// Gather f_i(x, t) for the cell (x, y) of the plane M.z0 from the post-collision array `fs`.
+// lo / hi: the plane below / above is a plate layer (half-way bounce-back).
+template <typename T, int LD>
+__device__ __forceinline__ void pull_map(const T* __restrict__ fs, const Geom& G, const PlaneMap& M,
+                                         int x, int y, bool lo, bool hi, Pop<T>& P) {
+  const size_t N = M.stride;
   const int nx = G.nx;
   const int xm = (x == 0) ? nx - 1 : x - 1;        // source column for e_x = +1
   const int xp = (x == nx - 1) ? 0 : x + 1;        // source column for e_x = -1
   const int ym = (y == 0) ? G.ny - 1 : y - 1;
   const int yp = (y == G.ny - 1) ? 0 : y + 1;
-  const unsigned r0 = (unsigned)z * G.plane + (unsigned)y * nx;    // own row
-  const unsigned rym = (unsigned)z * G.plane + (unsigned)ym * nx;  // row y-1, same z
-  const unsigned ryp = (unsigned)z * G.plane + (unsigned)yp * nx;
+  const unsigned o0 = (unsigned)y * nx, om = (unsigned)ym * nx, op = (unsigned)yp * nx;
+  const unsigned r0 = M.z0 + o0;                   // own row
+  const unsigned rym = M.z0 + om;                  // row y-1, same z
+  const unsigned ryp = M.z0 + op;
   const unsigned c = r0 + x;
-  const bool lo = (z == 1);           // z-1 is the bottom plate
-  const bool hi = (z == G.nz - 2);    // z+1 is the top plate
 
-  P.f[0] = ldg_stream(fs + c);
-  P.f[1] = ldg_stream(fs + 1 * N + r0 + xm);
-  P.f[2] = ldg_stream(fs + 2 * N + r0 + xp);
-  P.f[3] = ldg_stream(fs + 3 * N + rym + x);
-  P.f[4] = ldg_stream(fs + 4 * N + ryp + x);
-  P.f[7] = ldg_stream(fs + 7 * N + rym + xm);
-  P.f[8] = ldg_stream(fs + 8 * N + ryp + xp);
-  P.f[9] = ldg_stream(fs + 9 * N + ryp + xm);
-  P.f[10] = ldg_stream(fs + 10 * N + rym + xp);
+  P.f[0] = ldp<T, LD>(fs + c);
+  P.f[1] = ldp<T, LD>(fs + 1 * N + r0 + xm);
+  P.f[2] = ldp<T, LD>(fs + 2 * N + r0 + xp);
+  P.f[3] = ldp<T, LD>(fs + 3 * N + rym + x);
+  P.f[4] = ldp<T, LD>(fs + 4 * N + ryp + x);
+  P.f[7] = ldp<T, LD>(fs + 7 * N + rym + xm);
+  P.f[8] = ldp<T, LD>(fs + 8 * N + ryp + xp);
+  P.f[9] = ldp<T, LD>(fs + 9 * N + ryp + xm);
+  P.f[10] = ldp<T, LD>(fs + 10 * N + rym + xp);
   // directions with e_z = +1 come from z-1; at z = 1 they bounce off the bottom plate:
   // f_i(x, t) = f*_ibar(x, t-1)
-  {
-    const unsigned dn = G.plane;  // one layer
-    P.f[5] = lo ? ldg_stream(fs + 6 * N + c) : ldg_stream(fs + 5 * N + c - dn);
-    P.f[11] = lo ? ldg_stream(fs + 12 * N + c) : ldg_stream(fs + 11 * N + r0 - dn + xm);
-    P.f[14] = lo ? ldg_stream(fs + 13 * N + c) : ldg_stream(fs + 14 * N + r0 - dn + xp);
-    P.f[15] = lo ? ldg_stream(fs + 16 * N + c) : ldg_stream(fs + 15 * N + rym - dn + x);
-    P.f[18] = lo ? ldg_stream(fs + 17 * N + c) : ldg_stream(fs + 18 * N + ryp - dn + x);
-    // directions with e_z = -1 come from z+1; at z = nz-2 they bounce off the top plate
-    P.f[6] = hi ? ldg_stream(fs + 5 * N + c) : ldg_stream(fs + 6 * N + c + dn);
-    P.f[12] = hi ? ldg_stream(fs + 11 * N + c) : ldg_stream(fs + 12 * N + r0 + dn + xp);
-    P.f[13] = hi ? ldg_stream(fs + 14 * N + c) : ldg_stream(fs + 13 * N + r0 + dn + xm);
-    P.f[16] = hi ? ldg_stream(fs + 15 * N + c) : ldg_stream(fs + 16 * N + ryp + dn + x);
-    P.f[17] = hi ? ldg_stream(fs + 18 * N + c) : ldg_stream(fs + 17 * N + rym + dn + x);
-  }
+  P.f[5] = lo ? ldp<T, LD>(fs + 6 * N + c) : ldp<T, LD>(fs + 5 * N + M.zm + o0 + x);
+  P.f[11] = lo ? ldp<T, LD>(fs + 12 * N + c) : ldp<T, LD>(fs + 11 * N + M.zm + o0 + xm);
+  P.f[14] = lo ? ldp<T, LD>(fs + 13 * N + c) : ldp<T, LD>(fs + 14 * N + M.zm + o0 + xp);
+  P.f[15] = lo ? ldp<T, LD>(fs + 16 * N + c) : ldp<T, LD>(fs + 15 * N + M.zm + om + x);
+  P.f[18] = lo ? ldp<T, LD>(fs + 17 * N + c) : ldp<T, LD>(fs + 18 * N + M.zm + op + x);
+  // directions with e_z = -1 come from z+1; at z = nz-2 they bounce off the top plate
+  P.f[6] = hi ? ldp<T, LD>(fs + 5 * N + c) : ldp<T, LD>(fs + 6 * N + M.zp + o0 + x);
+  P.f[12] = hi ? ldp<T, LD>(fs + 11 * N + c) : ldp<T, LD>(fs + 12 * N + M.zp + o0 + xp);
+  P.f[13] = hi ? ldp<T, LD>(fs + 14 * N + c) : ldp<T, LD>(fs + 13 * N + M.zp + o0 + xm);
+  P.f[16] = hi ? ldp<T, LD>(fs + 15 * N + c) : ldp<T, LD>(fs + 16 * N + M.zp + op + x);
+  P.f[17] = hi ? ldp<T, LD>(fs + 18 * N + c) : ldp<T, LD>(fs + 17 * N + M.zp + om + x);
+}
+
+// The same for a cell (x, y, z) of a lattice array.
+template <typename T>
+__device__ __forceinline__ void pull(const T* __restrict__ fs, const Geom& G, int x, int y, int z,
+                                     Pop<T>& P) {
+  pull_map<T, LD_NC>(fs, G, lattice_map(G, z), x, y, z == 1, z == G.nz - 2, P);
 }
 
 // Moments.  Shifted: drho = sum f (Eq. 20), rho = 1 + drho; unshifted: rho = sum f (Eq. 16).
@@ -105,23 +138,26 @@ __device__ __forceinline__ void moments(const Pop<T>& P, T& drho, T& rho, T& jx,
   jz = (f[5] - f[6]) + (((f[11] - f[12]) - (f[13] - f[14])) + ((f[15] - f[16]) - (f[17] - f[18])));
 }
 
-// Collide one opposite pair (a: direction e, b: direction -e).
+// Collision of one cell, grouped so that every opposite pair shares its even and odd parts:
 //   f^eq,s = w [drho + rho (3 eu + 4.5 eu^2 - 1.5 u^2)]            Eq. 22 (never forms w + small)
 //   f^eq   = w rho [1 + 3 eu + 4.5 eu^2 - 1.5 u^2]                 Eq. 15
 //   S      = w [3 eF + 9 eu eF - 3 uF]                             Eq. 18 with c_s^2 = 1/3
 //   f*     = f - (f - f^eq)/tau + (1 - 1/(2 tau)) S                Eqs. 14 / 23
-template <typename T, bool SHIFTED>
-__device__ __forceinline__ void collide_pair(T& fa, T& fb, T w, T eu, T eF, T base, T rho, T sbase,
-                                             const LbConst<T>& C) {
-  // base = SHIFTED ? drho - 1.5 rho u^2 : rho (1 - 1.5 u^2);  sbase = -3 uF
-  const T even = base + T(4.5) * rho * eu * eu;
-  const T odd = T(3) * rho * eu;
-  const T seven = sbase + T(9) * eu * eF;
-  const T sodd = T(3) * eF;
-  const T feq_a = w * (even + odd), feq_b = w * (even - odd);
-  const T S_a = w * (seven + sodd), S_b = w * (seven - sodd);
-  fa = fa - C.omega * (fa - feq_a) + C.somega * S_a;
-  fb = fb - C.omega * (fb - feq_b) + C.somega * S_b;
+// With omega = 1/tau, s = 1 - omega/2, base = drho - 1.5 rho u^2 (shifted) or rho - 1.5 rho u^2:
+//   f*_(+-e) = (1 - omega) f_(+-e) + E +- O
+//   E = w [omega base - 3 s uF] + eu (4.5 w omega rho eu + 9 w s eF)     even in e
+//   O = 3 w omega rho eu + 3 w s eF                                       odd in e
+// (same terms as Eq. 23, summed in this fixed order.)
+template <typename T>
+struct PairConst { T k0, a, b3, c, d; };   // k0 = w(omega base - 3 s uF), a = 4.5 w omega rho, c = 3 w omega rho, d = 3 w s, b3 = 3 d
+
+template <typename T>
+__device__ __forceinline__ void collide_pair(T& fa, T& fb, T eu, T eF, const PairConst<T>& K, T keep) {
+  const T m = K.d * eF;                       // 3 w s eF
+  const T E = fmaf_t(eu, fmaf_t(K.a, eu, K.b3 * eF), K.k0);
+  const T O = fmaf_t(K.c, eu, m);
+  fa = fmaf_t(keep, fa, E + O);
+  fb = fmaf_t(keep, fb, E - O);
 }
 
 template <typename T, bool SHIFTED>
@@ -135,19 +171,24 @@ __device__ __forceinline__ void collide(Pop<T>& P, T Flx, T Fly, T Flz, const Lb
   const T u2 = ux * ux + uy * uy + uz * uz;
   const T uF = ux * Fx + uy * Fy + uz * Fz;
   const T base = SHIFTED ? drho - T(1.5) * rho * u2 : rho - T(1.5) * rho * u2;
-  const T sbase = T(-3) * uF;
+  const T keep = T(1) - C.omega;
+  const T t0 = C.omega * base - (T(3) * C.somega) * uF;   // omega base + s (-3 uF)
+  const T orho = C.omega * rho;
   const T w0 = T(1) / T(3), w1 = T(1) / T(18), w2 = T(1) / T(36);
+  PairConst<T> K1, K2;
+  K1.k0 = w1 * t0; K1.a = (T(4.5) * w1) * orho; K1.c = (T(3) * w1) * orho; K1.d = (T(3) * w1) * C.somega; K1.b3 = (T(9) * w1) * C.somega;
+  K2.k0 = w2 * t0; K2.a = (T(4.5) * w2) * orho; K2.c = (T(3) * w2) * orho; K2.d = (T(3) * w2) * C.somega; K2.b3 = (T(9) * w2) * C.somega;
   T* f = P.f;
-  f[0] = f[0] - C.omega * (f[0] - w0 * base) + C.somega * (w0 * sbase);
-  collide_pair<T, SHIFTED>(f[1], f[2], w1, ux, Fx, base, rho, sbase, C);
-  collide_pair<T, SHIFTED>(f[3], f[4], w1, uy, Fy, base, rho, sbase, C);
-  collide_pair<T, SHIFTED>(f[5], f[6], w1, uz, Fz, base, rho, sbase, C);
-  collide_pair<T, SHIFTED>(f[7], f[8], w2, ux + uy, Fx + Fy, base, rho, sbase, C);
-  collide_pair<T, SHIFTED>(f[9], f[10], w2, ux - uy, Fx - Fy, base, rho, sbase, C);
-  collide_pair<T, SHIFTED>(f[11], f[12], w2, ux + uz, Fx + Fz, base, rho, sbase, C);
-  collide_pair<T, SHIFTED>(f[13], f[14], w2, ux - uz, Fx - Fz, base, rho, sbase, C);
-  collide_pair<T, SHIFTED>(f[15], f[16], w2, uy + uz, Fy + Fz, base, rho, sbase, C);
-  collide_pair<T, SHIFTED>(f[17], f[18], w2, uy - uz, Fy - Fz, base, rho, sbase, C);
+  f[0] = fmaf_t(keep, f[0], w0 * t0);
+  collide_pair<T>(f[1], f[2], ux, Fx, K1, keep);
+  collide_pair<T>(f[3], f[4], uy, Fy, K1, keep);
+  collide_pair<T>(f[5], f[6], uz, Fz, K1, keep);
+  collide_pair<T>(f[7], f[8], ux + uy, Fx + Fy, K2, keep);
+  collide_pair<T>(f[9], f[10], ux - uy, Fx - Fy, K2, keep);
+  collide_pair<T>(f[11], f[12], ux + uz, Fx + Fz, K2, keep);
+  collide_pair<T>(f[13], f[14], ux - uz, Fx - Fz, K2, keep);
+  collide_pair<T>(f[15], f[16], uy + uz, Fy + Fz, K2, keep);
+  collide_pair<T>(f[17], f[18], uy - uz, Fy - Fz, K2, keep);
 }
 
 __device__ __forceinline__ void cell_of(unsigned fluid_index, const Geom& G, int& x, int& y, int& z) {

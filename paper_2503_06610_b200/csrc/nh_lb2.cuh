@@ -1,0 +1,317 @@
+// nh_lb2.cuh -- TWO lattice-Boltzmann steps per pass over HBM (temporal blocking through the L2).
+//
+// Same arithmetic as nh_lb.cuh, cell by cell and bit by bit (the same moments<> and collide<>):
+// PAPER.md:118-166, Eqs. 14-23; bounce-back PAPER.md:141; periodic x, y PAPER.md:225.
+// Between two director updates the force is frozen, so consecutive LB steps
+// depend on each other only through the populations, and two of them can share one sweep:
+//
+//   phase 1, plane k:  f*(t)   = collide(gather(A))      A  = lattice array in HBM (read once)
+//                      -> ring slot k mod R              the ring holds R z-planes and stays in L2
+//   phase 2, plane k:  f*(t+1) = collide(gather(ring))   needs ring planes k-1, k, k+1
+//                      -> B                              B  = the other lattice array (written once)
+//
+// One launch runs both phases as a wavefront along z.
+//   Unit of work: one PIECE (256*U consecutive cells: whole rows, or a whole fraction of a row) of
+//   one plane of one phase.  Units are ordered -- phase 1 of planes 0..D, then phase 2 of plane k
+//   and phase 1 of plane k+D+1 alternating, piece by piece inside a plane -- and persistent CTAs
+//   draw them from an atomic ticket counter (the next ticket is fetched while the current unit is
+//   worked on).
+//   Dependencies are per-piece flags in global memory holding the launch number:
+//     phase 2 of (k, piece)  needs phase 1 of planes k-1, k, k+1 at the 3x3 neighbouring pieces
+//     phase 1 of (k, piece)  needs phase 2 of planes k-R-1 .. k-R+1 at the same pieces (the readers
+//                            of the ring slot it overwrites)
+//   Every unit depends only on units EARLIER in ticket order and a CTA holds at most one unfinished
+//   unit, so the earliest unfinished unit can always proceed: no deadlock, no cooperative launch.
+//   A wait longer than ~4 s sets an error flag instead of hanging the device.
+//   Per unit a CTA meets at ONE barrier (all stores issued; next ticket and its readiness known);
+//   thread 0 then publishes the unit with a store-release while the other warps go on.
+//
+// Each thread updates U cells 32 apart in x, so the address arithmetic is shared between them.
+// DRAM traffic per cell and PAIR of steps: 19 words read + 19 written (+ F^LC), against 2 x that
+// for two single launches; the ring traffic (19 written + 19 read) stays in the 126 MB L2.
+#pragma once
+#include <cuda_runtime.h>
+#include "nh_lb.cuh"
+
+namespace nh {
+
+
+struct Wave {
+  unsigned long long* ticket;     // device counter, never reset
+  unsigned* flag1;                // [nzf][cps] launch number of the last finished phase-1 unit
+  unsigned* flag2;                // the same for phase 2
+  int* err;                       // set to 1 if a wait timed out
+  unsigned long long ticket_base; // value of *ticket when this launch starts
+  unsigned epoch;                 // this launch's number (> 0)
+  int nzf;                        // fluid planes
+  unsigned cps;                   // pieces per plane = prows * ppr
+  unsigned prows, ppr;            // piece grid: piece rows, pieces per piece row
+  unsigned rows_per_piece;        // lattice rows of one piece (1 when a row holds several pieces)
+  int spr_shift;                  // log2(32*U-cell segments of one piece that lie in one lattice row)
+  int D;                          // lead of phase 1 over phase 2, in planes (>= 1)
+  int R;                          // ring slots (planes), R >= D + 2
+  int reverse;                    // sweep from the top plate down
+  int dbg;
+};
+
+// p[i] = start of direction i inside a population array
+template <typename T> struct DirTab { T* p[Q]; };
+
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
+  unsigned v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Unit m of the launch order -> (phase, logical plane k).
+__device__ __forceinline__ void unit_of(unsigned m, int nzf, int D, int& phase, int& k) {
+  const int lead = min(D + 1, nzf);            // phase-1 planes before the first phase-2 plane
+  if ((int)m < lead) { phase = 1; k = (int)m; return; }
+  const int q = (int)m - lead;
+  const int pairs = nzf - lead;                // phase-1 planes left to interleave
+  if (q < 2 * pairs) {
+    if (q & 1) { phase = 1; k = lead + (q >> 1); }
+    else       { phase = 2; k = q >> 1; }
+    return;
+  }
+  phase = 2;
+  k = pairs + (q - 2 * pairs);
+}
+
+// What a unit is, decoded once by thread 0 and handed to the CTA through shared memory.
+struct UnitInfo {
+  unsigned ticket;     // >= total: no more work
+  int phase, k;
+  unsigned prow, q;    // position in the piece grid
+  int ready;           // dependencies were seen complete by the prefetching warp
+};
+
+// 27 flags a unit depends on (3 planes x 3x3 pieces, periodic in the piece grid): lane l < 27
+// looks at one of them.  deps_look issues the acquire load and returns the flag (or "done" where
+// there is nothing to wait for); deps_test is the vote over the warp.
+__device__ __forceinline__ unsigned deps_look(const Wave& W, int phase, int k, unsigned prow, unsigned q,
+                                              unsigned lane) {
+  unsigned v = 0xffffffffu;
+  if (lane < 27 && !(W.dbg & 2)) {
+    const int j = (phase == 2 ? k - 1 : k - W.R - 1) + (int)(lane / 9);
+    if (j >= 0 && j < W.nzf) {
+      const unsigned r9 = lane % 9, dr = r9 / 3, dq = r9 % 3;      // 0, 1, 2 -> -1, 0, +1
+      const unsigned pr = (prow + W.prows + dr - 1) % W.prows;
+      const unsigned pq = (q + W.ppr + dq - 1) % W.ppr;
+      v = ld_acquire_u32((phase == 2 ? W.flag1 : W.flag2) + (size_t)j * W.cps + pr * W.ppr + pq);
+    }
+  }
+  return v;
+}
+__device__ __forceinline__ bool deps_test(const Wave& W, unsigned v) { return __all_sync(0xffffffffu, v >= W.epoch); }
+__device__ __forceinline__ bool deps_ready(const Wave& W, int phase, int k, unsigned prow, unsigned q,
+                                           unsigned lane) {
+  return deps_test(W, deps_look(W, phase, k, prow, q, lane));
+}
+
+// f_i(x, t) = f*_i(x - e_i, t-1) with half-way bounce-back for the U cells (xA + 32 j, y) of one
+// thread.  zm, z0, zp: element offsets of the planes z-1, z, z+1 inside each direction's array;
+// r0, rm, rp: offsets of the rows y, y-1, y+1 (periodic) inside a plane.  lo / hi: the plane
+// below / above is a plate.  Directions as in nh_lb.cuh.
+template <typename T, int LD, int U, typename Tab>
+__device__ __forceinline__ void gather_cells(const Tab& S, unsigned zm, unsigned z0, unsigned zp,
+                                             unsigned r0, unsigned rm, unsigned rp, unsigned xA,
+                                             unsigned nx, bool lo, bool hi, Pop<T> (&P)[U]) {
+  unsigned xm[U], xp[U];        // source columns for e_x = +1 / -1
+#pragma unroll
+  for (int j = 0; j < U; ++j) {
+    const unsigned x = xA + 32u * j;
+    xm[j] = (x == 0) ? nx - 1 : x - 1;
+    xp[j] = (x == nx - 1) ? 0u : x + 1;
+  }
+  // e_x = 0: one address, the U cells are 32 elements apart
+#define NH_SAME(i, src, off)                                            \
+  {                                                                     \
+    const T* q_ = S.p[src] + ((off) + xA);                              \
+    _Pragma("unroll") for (int j = 0; j < U; ++j) P[j].f[i] = ldp<T, LD>(q_ + 32 * j); \
+  }
+#define NH_SHIFT(i, src, off, xs)                                       \
+  {                                                                     \
+    _Pragma("unroll") for (int j = 0; j < U; ++j) P[j].f[i] = ldp<T, LD>(S.p[src] + ((off) + xs[j])); \
+  }
+  const unsigned own = z0 + r0;
+  NH_SAME(0, 0, own)
+  NH_SHIFT(1, 1, own, xm)
+  NH_SHIFT(2, 2, own, xp)
+  NH_SAME(3, 3, z0 + rm)
+  NH_SAME(4, 4, z0 + rp)
+  NH_SHIFT(7, 7, z0 + rm, xm)
+  NH_SHIFT(8, 8, z0 + rp, xp)
+  NH_SHIFT(9, 9, z0 + rp, xm)
+  NH_SHIFT(10, 10, z0 + rm, xp)
+  if (lo) {   // e_z = +1 would come out of the bottom plate: the opposite direction at the own cell
+    NH_SAME(5, 6, own)
+    NH_SAME(11, 12, own)
+    NH_SAME(14, 13, own)
+    NH_SAME(15, 16, own)
+    NH_SAME(18, 17, own)
+  } else {
+    NH_SAME(5, 5, zm + r0)
+    NH_SHIFT(11, 11, zm + r0, xm)
+    NH_SHIFT(14, 14, zm + r0, xp)
+    NH_SAME(15, 15, zm + rm)
+    NH_SAME(18, 18, zm + rp)
+  }
+  if (hi) {   // e_z = -1 would come out of the top plate
+    NH_SAME(6, 5, own)
+    NH_SAME(12, 11, own)
+    NH_SAME(13, 14, own)
+    NH_SAME(16, 15, own)
+    NH_SAME(17, 18, own)
+  } else {
+    NH_SAME(6, 6, zp + r0)
+    NH_SHIFT(12, 12, zp + r0, xp)
+    NH_SHIFT(13, 13, zp + r0, xm)
+    NH_SAME(16, 16, zp + rp)
+    NH_SAME(17, 17, zp + rm)
+  }
+#undef NH_SAME
+#undef NH_SHIFT
+}
+
+// Per unit a CTA meets at ONE barrier (all stores issued; the next unit and its readiness known);
+// thread 0 then publishes the unit with a store-release while the other warps go on.  Warp 0 looks
+// at the flags of the NEXT unit while its loads of the current one are in flight.
+template <typename T, bool SHIFTED, int U, int NT>
+__global__ void __launch_bounds__(NT, (sizeof(T) == 4 ? (U == 2 ? 3 : 4) : (U == 2 ? 1 : 2)) * (256 / NT))
+lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restrict__ Flc,
+               Geom G, LbConst<T> C, Wave W) {
+  __shared__ UnitInfo s_info[3];
+  const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  const unsigned total = 2u * (unsigned)W.nzf * W.cps;
+
+  auto decode = [&](unsigned tk, UnitInfo& I) {
+    I.ticket = tk;
+    I.ready = 0;
+    if (tk < total) {
+      const unsigned unit = tk / W.cps, piece = tk - unit * W.cps;
+      unit_of(unit, W.nzf, W.D, I.phase, I.k);
+      I.prow = piece / W.ppr;
+      I.q = piece - I.prow * W.ppr;
+    }
+  };
+  // thread 0 keeps three tickets ahead: this unit and the next are decoded in shared memory when
+  // a unit starts (so the next one can be warmed and looked at), the one after that is decoded
+  // while this one is worked on, and a fourth ticket is in flight
+  unsigned long long tnext = 0;
+  if (threadIdx.x == 0) {
+    decode((unsigned)(atomicAdd(W.ticket, 1ull) - W.ticket_base), s_info[0]);
+    decode((unsigned)(atomicAdd(W.ticket, 1ull) - W.ticket_base), s_info[1]);
+    tnext = atomicAdd(W.ticket, 1ull);
+  }
+  __syncthreads();
+
+  // this thread's place inside a piece
+  const unsigned seg_row = warp >> W.spr_shift;                             // lattice row inside the piece
+  const unsigned seg_x = (warp & ((1u << W.spr_shift) - 1u)) * (32u * U);   // first column of the warp's segment
+  unsigned b0 = 0;
+  for (;;) {
+    const unsigned b1 = (b0 == 2 ? 0u : b0 + 1), b2 = (b1 == 2 ? 0u : b1 + 1);
+    const UnitInfo I = s_info[b0];
+    if (I.ticket >= total) break;
+    const UnitInfo Nx = s_info[b1];
+    if (threadIdx.x == 0) {
+      decode((unsigned)(tnext - W.ticket_base), s_info[b2]);
+      tnext = atomicAdd(W.ticket, 1ull);                        // consumed one unit later
+    }
+    if (!I.ready) {
+      const long long t0 = clock64();
+      unsigned ns = 32;
+      while (!deps_ready(W, I.phase, I.k, I.prow, I.q, lane)) {
+        __nanosleep(ns);
+        if (ns < 512) ns *= 2;
+        if (clock64() - t0 > 8000000000ll) { if (lane == 0) atomicExch(W.err, 1); break; }
+      }
+    }
+
+    const int z = (W.reverse ? W.nzf - 1 - I.k : I.k) + 1;                  // physical plane
+    const unsigned y = I.prow * W.rows_per_piece + seg_row;
+    const unsigned xA = I.q * (unsigned)(NT * U) + seg_x + lane;
+    const bool active = y < (unsigned)G.ny && !((W.dbg & 8) && I.phase == 2) && !((W.dbg & 16) && I.phase == 1);
+    const unsigned nx = (unsigned)G.nx;
+    const unsigned r0 = y * nx;
+    const unsigned slot = (unsigned)((z - 1) % W.R);
+    const unsigned cell = (unsigned)z * G.plane + r0 + xA;
+    Pop<T> P[U];
+    T Fx[U], Fy[U], Fz[U];
+    if (active) {
+      const unsigned rm = (y == 0 ? (unsigned)G.ny - 1 : y - 1) * nx;
+      const unsigned rp = (y == (unsigned)G.ny - 1 ? 0u : y + 1) * nx;
+      const bool lo = (z == 1), hi = (z == G.nz - 2);
+      if (I.phase == 1) {
+        const unsigned z0 = (unsigned)z * G.plane;
+        gather_cells<T, LD_CS, U>(A, z0 - G.plane, z0, z0 + G.plane, r0, rm, rp, xA, nx, lo, hi, P);
+      } else {
+        const unsigned sm = (slot == 0 ? (unsigned)W.R - 1 : slot - 1), sp = (slot == (unsigned)W.R - 1 ? 0u : slot + 1);
+        gather_cells<T, LD_CG, U>(ring, sm * G.plane, slot * G.plane, sp * G.plane, r0, rm, rp, xA, nx, lo, hi, P);
+      }
+#pragma unroll
+      for (int j = 0; j < U; ++j) {
+        Fx[j] = Fy[j] = Fz[j] = T(0);
+        if (C.use_flc) {
+          const T* f = Flc + cell;
+          Fx[j] = __ldg(f + 32 * j); Fy[j] = __ldg(f + G.N + 32 * j); Fz[j] = __ldg(f + 2 * G.N + 32 * j);
+        }
+      }
+    }
+    // warm the L2 with what this thread will gather from HBM in the next unit (phase 1 only: a
+    // phase-2 unit reads the ring, which is in the L2 already)
+    if (Nx.ticket < total && Nx.phase == 1 && !(W.dbg & 4)) {
+      const int zn = (W.reverse ? W.nzf - 1 - Nx.k : Nx.k) + 1;
+      const unsigned yn = Nx.prow * W.rows_per_piece + seg_row;
+      if (yn < (unsigned)G.ny) {
+        const unsigned xn = Nx.q * (unsigned)(NT * U) + seg_x + lane;
+        const unsigned rn0 = yn * nx;
+        const unsigned rnm = (yn == 0 ? (unsigned)G.ny - 1 : yn - 1) * nx;
+        const unsigned rnp = (yn == (unsigned)G.ny - 1 ? 0u : yn + 1) * nx;
+        const unsigned z0 = (unsigned)zn * G.plane;
+        Pop<T> dummy[U];
+        gather_cells<T, LD_PF, U>(A, z0 - G.plane, z0, z0 + G.plane, rn0, rnm, rnp, xn, nx, zn == 1, zn == G.nz - 2, dummy);
+      }
+    }
+    // warp 0: a look (not a wait: this unit is not published yet) at the flags of the next unit; the
+    // answer is needed only after this unit's stores, so its latency hides under the work
+    unsigned look = 0;
+    if (warp == 0 && Nx.ticket < total) look = deps_look(W, Nx.phase, Nx.k, Nx.prow, Nx.q, lane);
+    if (active) {
+#pragma unroll
+      for (int j = 0; j < U; ++j) collide<T, SHIFTED>(P[j], Fx[j], Fy[j], Fz[j], C);
+      if (I.phase == 1) {
+        const unsigned o = slot * G.plane + r0 + xA;
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+          T* d = ring.p[i] + o;
+#pragma unroll
+          for (int j = 0; j < U; ++j) d[32 * j] = P[j].f[i];
+        }
+      } else {
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+          T* d = B.p[i] + cell;
+#pragma unroll
+          for (int j = 0; j < U; ++j) __stcs(d + 32 * j, P[j].f[i]);
+        }
+      }
+    }
+    if (warp == 0) {
+      const bool ok = deps_test(W, look);
+      if (lane == 0) s_info[b1].ready = (ok && Nx.ticket < total) ? 1 : 0;
+    }
+    __syncthreads();      // every store of this unit is issued; s_info[b1], s_info[b2] are complete
+    if (threadIdx.x == 0) {
+      unsigned* f = (I.phase == 1 ? W.flag1 : W.flag2) + (size_t)I.k * W.cps + I.prow * W.ppr + I.q;
+      if (W.dbg & 1) *(volatile unsigned*)f = W.epoch; else st_release_u32(f, W.epoch);
+    }
+    b0 = b1;
+  }
+}
+
+}  // namespace nh

@@ -211,3 +211,35 @@ def test_options_do_not_change_results():
             assert cnt == 81 and ms > 0.0
             assert g.kernel_time("predictor")[1] == 27
         assert g.launch_count > 81
+
+
+@pytest.mark.parametrize("shape,r", [((64, 64, 32), 10), ((128, 5, 20), 7), ((32, 7, 9), 3), ((512, 4, 6), 2),
+                                     ((1024, 3, 5), 2), ((64, 3, 3), 2), ((256, 9, 8), 4), ((16, 16, 8), 1)])
+def test_two_step_kernel_is_bit_identical(shape, r):
+    """The two-steps-per-sweep LB kernel (L2-resident plane ring, wavefront along z) does the same
+    arithmetic per cell as the one-step kernel, so every field must agree bit for bit, whatever
+    the lead / ring size / CTA shape, for uneven step() chunks and odd FD ratios; grids that do
+    not tile into pieces (16 wide) silently take the one-step kernel."""
+    m = nh()
+    nx, ny, nz = shape
+    d = I.noisy_homeotropic(nx, ny, nz, 0.1)
+    p = dict(nx=nx, ny=ny, nz=nz, tau=0.7, K=0.015, pitch=9.0, xi=0.8, gamma1=1.3, g=(2e-6, -1e-6, 0.0), fd_ratio=r)
+
+    def run(precision, opt, chunks):
+        g = m.Lattice(**dict(p, precision=precision))
+        g.set_options(opt)
+        g.set_director(d)
+        for c in chunks:
+            g.step(c)
+        f = g.get_fields()
+        g.close()
+        return f
+
+    T = m.OPT_LB_TWOSTEP
+    for precision in (0, 1):
+        ref = run(precision, 0, [43])
+        for opt in (T, T | m.OPT_NO_SERPENTINE, T | (1 << 30), T | (1 << 31), T | (1 << 16) | (3 << 20),
+                    T | (3 << 16) | (12 << 20) | (2 << 26)):
+            f = run(precision, opt, [1, 7, 20, 15])
+            for k in ref:
+                assert np.array_equal(ref[k], f[k]), (shape, precision, hex(opt), k)
