@@ -39,7 +39,8 @@ def parse():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--precision", default="fp32s", choices=sorted(PRECISIONS))
     ap.add_argument("--size", type=int, nargs=3, default=None, help="configs[4] grid (nx ny nz)")
-    ap.add_argument("--options", type=int, default=0, help="nh_set_options bits (kernel variants)")
+    ap.add_argument("--options", type=lambda v: int(v, 0), default=0, help="nh_set_options bits (kernel variants)")
+    ap.add_argument("--two-step", action="store_true", help="NH_OPT_LB_TWOSTEP: two LB steps per launch through the L2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -217,7 +218,7 @@ def main():
     lat = nh.Lattice(device="cuda:%d" % local, **dict(p, precision=prec))
     d_pinned = torch.from_numpy(d).pin_memory()
     lat.set_director(d_pinned)
-    base_opt = args.options
+    base_opt = args.options | (nh.OPT_LB_TWOSTEP if args.two_step else 0)
 
     def barrier():
         torch.cuda.synchronize()
@@ -259,15 +260,22 @@ def main():
         lat.step(r)
     kt = {k: lat.kernel_time(k) for k in nh.KERNEL_CLASSES}
     lat.set_options(base_opt)
-    lb_ms, lb_n = kt["lb"]
+    # dominant kernel: the one-step LB launch, or the two-step launch (2 LB steps each) when it is on
+    two = kt["lb2"][0] > kt["lb"][0]
+    lb_ms, lb_n = kt["lb2"] if two else kt["lb"]
+    steps_per_launch = 2 if two else 1
     lb_avg = lb_ms / max(lb_n, 1)
     total_k = sum(v[0] for v in kt.values())
     peak, peak_src = peaks()
-    alg_bytes = 41 * word * nf          # 19 read + 19 write + 3 (F^LC) words per fluid cell
+    # 19 read + 19 write + 3 (F^LC) words per fluid cell and LB step
+    alg_bytes = 41 * word * nf * steps_per_launch
     achieved = alg_bytes / (lb_avg * 1e-3) / 1e9 if lb_avg > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "lb_step (collide+stream+force)", "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(args.precision, desc["grid"]),
+    kname = "lb_wave (2 x collide+stream+force per launch)" if two else "lb_step (collide+stream+force)"
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak,
+                "traffic": ncu_traffic(args.precision + ("+2step" if two else ""), desc["grid"]),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
+                "lb_steps_per_launch": steps_per_launch,
                 "avg_launch_ms": lb_avg, "launches_timed": lb_n, "share_of_step": lb_ms / total_k if total_k else None,
                 "kernel_ms": {k: round(v[0], 4) for k, v in kt.items()},
                 "full_step_bytes_per_cell": (41 + 30.0 / r) * word,

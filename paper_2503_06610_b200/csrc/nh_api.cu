@@ -9,7 +9,6 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
-#include <cstdlib>
 #include <new>
 #include <string>
 #include <vector>
@@ -94,7 +93,7 @@ struct nh_lattice {
   int ring_cap;     // planes it holds
   unsigned long long* wave;   // device counters of the two-step kernel: err flag at [4], done1, done2 from [8]
   unsigned long long wave_epoch, wave_tickets;
-  int sm_count, wave_ctas_per_sm;
+  int sm_count;
   // per-class CUDA-event timing (option bit1)
   struct Pair { cudaEvent_t a, b; int cls; };
   std::vector<Pair> pool;
@@ -240,13 +239,12 @@ int launch_lb2_u(nh_lattice* L) {
   W.flag2 = W.flag1 + (size_t)nzf * W.cps;
   W.nzf = nzf;
   int D = (L->options >> 16) & 0xf, R = (L->options >> 20) & 0x3f;
-  if (D == 0) D = 4;
-  if (R == 0) R = D + 6;
+  if (D == 0) D = 5;
+  if (R == 0) R = D + 7;
   if (R > L->ring_cap) R = L->ring_cap;
   if (D > R - 2) D = R - 2;
   W.D = D; W.R = R;
   W.reverse = next_sweep(L);
-  { const char* e = getenv("NH_WAVE_DBG"); W.dbg = e ? atoi(e) : 0; }
   const unsigned long long units = 2ull * nzf * W.cps;
   int per_sm_max = 0;
   NH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_max, nh::lb_wave_kernel<T, SH, U, NT>, NT, 0));

@@ -47,14 +47,12 @@ __device__ __forceinline__ double fmaf_t(double a, double b, double c) { return 
 // Load policies of the gathers: LD_NC read-only path (data not written during the launch),
 // LD_CS the same with the streaming (evict-first) hint, LD_CG coherent at L2 (data that another CTA
 // of the SAME launch has written: the ring of the two-step kernel, nh_lb2.cuh).
-// LD_PF loads nothing: it asks the L2 to fetch the line (the two-step kernel warms the next unit).
-enum { LD_NC = 0, LD_CS = 1, LD_CG = 2, LD_PF = 3 };
+enum { LD_NC = 0, LD_CS = 1, LD_CG = 2 };
 template <typename T, int LD>
 __device__ __forceinline__ T ldp(const T* p) {
   if constexpr (LD == LD_NC) return __ldg(p);
   else if constexpr (LD == LD_CS) return __ldcs(p);
-  else if constexpr (LD == LD_CG) return __ldcg(p);
-  else { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); return T(0); }
+  else return __ldcg(p);
 }
 
 // Where the three z planes a gather touches live inside a population array: element offsets of
@@ -209,7 +207,7 @@ __device__ __forceinline__ unsigned sweep_block(int reverse) {
 
 // One LB step, one thread per fluid cell (baseline variant; nh_lb_vec.cuh holds the wide one).
 template <typename T, bool SHIFTED>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, sizeof(T) == 4 ? 6 : 3)
 lb_step_kernel(const T* __restrict__ fsrc, T* __restrict__ fdst, const T* __restrict__ Flc,
                Geom G, LbConst<T> C, int reverse) {
   const unsigned k = sweep_block(reverse) * blockDim.x + threadIdx.x;

@@ -51,7 +51,6 @@ struct Wave {
   int D;                          // lead of phase 1 over phase 2, in planes (>= 1)
   int R;                          // ring slots (planes), R >= D + 2
   int reverse;                    // sweep from the top plate down
-  int dbg;
 };
 
 // p[i] = start of direction i inside a population array
@@ -95,7 +94,7 @@ struct UnitInfo {
 __device__ __forceinline__ unsigned deps_look(const Wave& W, int phase, int k, unsigned prow, unsigned q,
                                               unsigned lane) {
   unsigned v = 0xffffffffu;
-  if (lane < 27 && !(W.dbg & 2)) {
+  if (lane < 27) {
     const int j = (phase == 2 ? k - 1 : k - W.R - 1) + (int)(lane / 9);
     if (j >= 0 && j < W.nzf) {
       const unsigned r9 = lane % 9, dr = r9 / 3, dq = r9 % 3;      // 0, 1, 2 -> -1, 0, +1
@@ -235,7 +234,7 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
     const int z = (W.reverse ? W.nzf - 1 - I.k : I.k) + 1;                  // physical plane
     const unsigned y = I.prow * W.rows_per_piece + seg_row;
     const unsigned xA = I.q * (unsigned)(NT * U) + seg_x + lane;
-    const bool active = y < (unsigned)G.ny && !((W.dbg & 8) && I.phase == 2) && !((W.dbg & 16) && I.phase == 1);
+    const bool active = y < (unsigned)G.ny;
     const unsigned nx = (unsigned)G.nx;
     const unsigned r0 = y * nx;
     const unsigned slot = (unsigned)((z - 1) % W.R);
@@ -260,21 +259,6 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
           const T* f = Flc + cell;
           Fx[j] = __ldg(f + 32 * j); Fy[j] = __ldg(f + G.N + 32 * j); Fz[j] = __ldg(f + 2 * G.N + 32 * j);
         }
-      }
-    }
-    // warm the L2 with what this thread will gather from HBM in the next unit (phase 1 only: a
-    // phase-2 unit reads the ring, which is in the L2 already)
-    if (Nx.ticket < total && Nx.phase == 1 && !(W.dbg & 4)) {
-      const int zn = (W.reverse ? W.nzf - 1 - Nx.k : Nx.k) + 1;
-      const unsigned yn = Nx.prow * W.rows_per_piece + seg_row;
-      if (yn < (unsigned)G.ny) {
-        const unsigned xn = Nx.q * (unsigned)(NT * U) + seg_x + lane;
-        const unsigned rn0 = yn * nx;
-        const unsigned rnm = (yn == 0 ? (unsigned)G.ny - 1 : yn - 1) * nx;
-        const unsigned rnp = (yn == (unsigned)G.ny - 1 ? 0u : yn + 1) * nx;
-        const unsigned z0 = (unsigned)zn * G.plane;
-        Pop<T> dummy[U];
-        gather_cells<T, LD_PF, U>(A, z0 - G.plane, z0, z0 + G.plane, rn0, rnm, rnp, xn, nx, zn == 1, zn == G.nz - 2, dummy);
       }
     }
     // warp 0: a look (not a wait: this unit is not published yet) at the flags of the next unit; the
@@ -308,7 +292,7 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
     __syncthreads();      // every store of this unit is issued; s_info[b1], s_info[b2] are complete
     if (threadIdx.x == 0) {
       unsigned* f = (I.phase == 1 ? W.flag1 : W.flag2) + (size_t)I.k * W.cps + I.prow * W.ppr + I.q;
-      if (W.dbg & 1) *(volatile unsigned*)f = W.epoch; else st_release_u32(f, W.epoch);
+      st_release_u32(f, W.epoch);
     }
     b0 = b1;
   }

@@ -243,3 +243,38 @@ def test_two_step_kernel_is_bit_identical(shape, r):
             f = run(precision, opt, [1, 7, 20, 15])
             for k in ref:
                 assert np.array_equal(ref[k], f[k]), (shape, precision, hex(opt), k)
+
+
+def test_config3_full_size_bench_configuration():
+    """BASELINE.json configs[3] at FULL size (256x256x64, two tubes, r = 10), in the launch
+    configurations bench.py times (default options, and the two-step LB kernel): FP64 within 1e-10
+    at 100 steps, shifted FP32 within (1e-3, 1e-4) at 100 and at 1000 steps (north_star's bar), every
+    output element compared with the oracle; the two-step run must equal the default FP32 run bit
+    for bit.  One oracle run (about 90 s of host time) serves all of them."""
+    m = nh()
+    p = I.config(3)
+    d = p.pop("director")
+    p.pop("steps")
+    o = Oracle(**dict(p, precision=0))
+    o.set_director(d)
+    g64 = m.Lattice(**dict(p, precision=0))
+    g32 = m.Lattice(**dict(p, precision=1))
+    g32w = m.Lattice(**dict(p, precision=1))
+    g32w.set_options(m.OPT_LB_TWOSTEP)
+    for g in (g64, g32, g32w):
+        g.set_director(d)
+    for n in (100, 900):
+        o.step(n)
+        for g in (g64, g32, g32w):
+            g.step(n)
+        if o.time == 100:
+            compare(o, g64, FP64_TOL, FP64_TOL, label="cfg3 full fp64")
+        compare(o, g32, FP32_TOL_U, FP32_TOL_N, tol_f=5e-3, label="cfg3 full fp32 shifted")
+        a, b = g32.get_fields(), g32w.get_fields()
+        for k in a:
+            assert np.array_equal(a[k], b[k]), k
+    assert g32w.kernel_time("lb2")[1] > 0 and g32.kernel_time("lb2")[1] == 0
+    f = g64.get_fields()
+    nf = p["nx"] * p["ny"] * (p["nz"] - 2)
+    assert abs((f["rho"][1:-1] - 1.0).sum()) / nf < 1e-12          # mass (pin P2) on the GPU at full size
+    assert np.abs(np.sqrt((f["n"] ** 2).sum(0)) - 1.0).max() < 1e-14
