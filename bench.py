@@ -186,6 +186,22 @@ def cpu_baseline(p, d, precision):
                       % (periods, periods * r, periods, p["nx"], p["ny"], p["nz"], dt)}
 
 
+def max_over_ranks(ms, world, device="cuda"):
+    """Step time of the job = the slowest rank's device time (replicas only: no data-path collective)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_mlups(world, fluid_cells, lb_steps, ms):
+    """Whole-job throughput: every rank advanced its own replica by lb_steps LB steps in ms."""
+    return world * fluid_cells * lb_steps / (ms * 1e-3) / 1e6
+
+
 def main():
     args = parse()
     if args.impl == "reference":
@@ -233,12 +249,7 @@ def main():
         fn()
         ev1.record()
         barrier()
-        ms = ev0.elapsed_time(ev1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return max_over_ranks(ev0.elapsed_time(ev1), world)
 
     # ---- device-resident timing: W warm-up steps, then exactly K steps ----------------------------
     lat.set_options(base_opt)
@@ -251,7 +262,7 @@ def main():
     ms = timed(lambda: [lat.step(r) for _ in range(args.steps)])
     launches = lat.launch_count - l0
     clocks = sampler.stop() if rank == 0 else None
-    mlups = world * nf * r * args.steps / (ms * 1e-3) / 1e6
+    mlups = job_mlups(world, nf, r * args.steps, ms)
 
     # ---- second pass of the same K steps with a CUDA-event pair around every launch ---------------
     lat.set_options(base_opt | nh.OPT_TIMING)
@@ -304,11 +315,11 @@ def main():
                 lat.get_fields(out=out, which=("u", "n"))
 
         ms_every = timed(every)
-        e2e = {"value": world * nf * r * args.steps / (ms_job * 1e-3) / 1e6, "unit": "MLUPS",
+        e2e = {"value": job_mlups(world, nf, r * args.steps, ms_job), "unit": "MLUPS",
                "h2d_bytes_per_step": 24 * N / args.steps, "d2h_bytes_per_step": 48 * N / args.steps,
                "what": "one job = nh_set_director(pinned host n) + K steps + nh_get_fields(u, n -> pinned host), "
                        "all inside the timed region; bytes are the job's copies divided by K",
-               "copies_every_step": {"value": world * nf * r * 3 / (ms_every * 1e-3) / 1e6, "unit": "MLUPS",
+               "copies_every_step": {"value": job_mlups(world, nf, r * 3, ms_every), "unit": "MLUPS",
                                      "h2d_bytes_per_step": 24 * N, "d2h_bytes_per_step": 48 * N}}
 
     if rank != 0:

@@ -100,7 +100,10 @@ long nh_time(const nh_lattice* L);
 long nh_launch_count(const nh_lattice* L);
 
 /* Options (results agree within round-off whatever they are):
- *   bit0 NH_OPT_GRAPH         replay nh_step through CUDA graphs (launch-bound small grids)
+ *   bit0 NH_OPT_GRAPH         replay nh_step through CUDA graphs (launch-bound small grids): one
+ *                             executable graph per distinct (n_lb, r, t mod r, buffer parity), captured
+ *                             on first use.  Needs a capturable stream (not the legacy default
+ *                             stream), otherwise plain launches; excludes NH_OPT_LB_TWOSTEP.
  *   bit1 NH_OPT_TIMING        bracket every kernel launch with a CUDA-event pair on the lattice's
  *                             stream (ignored while graphs are on)
  *   bit2 NH_OPT_FD_DIRECT     use the one-thread-per-cell FD kernels instead of the tiled ones

@@ -94,6 +94,14 @@ struct nh_lattice {
   unsigned long long* wave;   // device counters of the two-step kernel: err flag at [4], done1, done2 from [8]
   unsigned long long wave_epoch, wave_tickets;
   int sm_count;
+  // CUDA-graph replay of nh_step (NH_OPT_GRAPH): one executable graph per distinct call shape
+  struct Graph {
+    int n_lb, r, phase, cur, ncur, sweep, options;   // key: arguments and the state the launches depend on
+    cudaGraphExec_t exec;
+    int cur_after, ncur_after, sweep_after;          // state after the call
+    long cnt[KC_COUNT];                              // launches per class
+  };
+  std::vector<Graph> graphs;
   // per-class CUDA-event timing (option bit1)
   struct Pair { cudaEvent_t a, b; int cls; };
   std::vector<Pair> pool;
@@ -129,7 +137,7 @@ struct Bracket {
   Bracket(nh_lattice* L_, int cls) : L(L_), slot(-1), rc(NH_OK) {
     L->launches += 1;
     L->cnt[cls] += 1;
-    if (!(L->options & 2)) return;
+    if (!(L->options & 2) || (L->options & NH_OPT_GRAPH)) return;
     if (L->used == L->pool.size()) {
       if (L->pool.size() >= 4096) { rc = drain_events(L); if (rc) return; }
       else {
@@ -220,7 +228,9 @@ int lb2_cells_per_thread(const nh_lattice* L) {
   return 0;
 }
 bool lb2_usable(const nh_lattice* L) {
-  return (L->options & NH_OPT_LB_TWOSTEP) && L->ring_cap >= 3 && lb2_cells_per_thread(L) > 0;
+  // (not under graph replay: a launch carries its own number and ticket base as arguments)
+  return (L->options & NH_OPT_LB_TWOSTEP) && !(L->options & NH_OPT_GRAPH) && L->ring_cap >= 3 &&
+         lb2_cells_per_thread(L) > 0;
 }
 
 template <typename T, bool SH, int U, int NT>
@@ -494,6 +504,10 @@ int get_fields_typed(nh_lattice* L, double* rho, double* u, double* n, double* F
   return NH_OK;
 }
 
+int step_plain(nh_lattice* L, int n_lb, int r);
+int step_graph(nh_lattice* L, int n_lb, int r);
+constexpr int NH_EAGAIN = 1;   // internal: fall back to plain launches
+
 #define NH_DISPATCH(L, CALL_F64S, CALL_F32S, CALL_F32U, CALL_F64U) \
   switch ((L)->p.precision) {                                      \
     case NH_FP64_SHIFTED: return CALL_F64S;                        \
@@ -501,6 +515,54 @@ int get_fields_typed(nh_lattice* L, double* rho, double* u, double* n, double* F
     case NH_FP32_UNSHIFTED: return CALL_F32U;                      \
     default: return CALL_F64U;                                     \
   }
+
+int step_plain(nh_lattice* L, int n_lb, int r) {
+  NH_DISPATCH(L, (step_typed<double, true>(L, n_lb, r)), (step_typed<float, true>(L, n_lb, r)),
+              (step_typed<float, false>(L, n_lb, r)), (step_typed<double, false>(L, n_lb, r)));
+}
+
+// Replay of one nh_step call through a CUDA graph.  The launch sequence of a call depends only on
+// (n_lb, r, t mod r) and on which ping-pong buffers and sweep direction it starts from, so the
+// captured graph of one call serves every later call with the same key.  The first call with a new
+// key captures the launches of step_plain on the lattice's stream (nothing runs during capture)
+// and then launches the graph once.
+int step_graph(nh_lattice* L, int n_lb, int r) {
+  nh_lattice::Graph key;
+  key.n_lb = n_lb; key.r = r; key.phase = r > 0 ? (int)(L->t % r) : 0;
+  key.cur = L->cur; key.ncur = L->ncur; key.sweep = L->sweep; key.options = L->options;
+  for (const auto& g : L->graphs) {
+    if (g.n_lb == key.n_lb && g.r == key.r && g.phase == key.phase && g.cur == key.cur && g.ncur == key.ncur &&
+        g.sweep == key.sweep && g.options == key.options) {
+      NH_CUDA(cudaGraphLaunch(g.exec, L->stream));
+      L->cur = g.cur_after; L->ncur = g.ncur_after; L->sweep = g.sweep_after;
+      L->t += n_lb;
+      for (int k = 0; k < KC_COUNT; ++k) { L->cnt[k] += g.cnt[k]; L->launches += g.cnt[k]; }
+      return NH_OK;
+    }
+  }
+  if (cudaStreamBeginCapture(L->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    cudaGetLastError();                       // e.g. the legacy default stream
+    return NH_EAGAIN;
+  }
+  long before[KC_COUNT];
+  for (int k = 0; k < KC_COUNT; ++k) before[k] = L->cnt[k];
+  const int rc = step_plain(L, n_lb, r);
+  cudaGraph_t graph = nullptr;
+  const cudaError_t e = cudaStreamEndCapture(L->stream, &graph);
+  if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+  if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+  cudaGraphExec_t exec = nullptr;
+  const cudaError_t e2 = cudaGraphInstantiate(&exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e2 != cudaSuccess) return cuda_fail(e2, "cudaGraphInstantiate");
+  NH_CUDA(cudaGraphLaunch(exec, L->stream));
+  key.exec = exec;
+  key.cur_after = L->cur; key.ncur_after = L->ncur; key.sweep_after = L->sweep;
+  for (int k = 0; k < KC_COUNT; ++k) key.cnt[k] = L->cnt[k] - before[k];
+  if (L->graphs.size() < 64) L->graphs.push_back(key);
+  else { NH_CUDA(cudaStreamSynchronize(L->stream)); cudaGraphExecDestroy(exec); }
+  return NH_OK;
+}
 
 }  // namespace
 
@@ -599,8 +661,11 @@ int nh_step(nh_lattice* L, int n_lb, int n_fd) {
   if (!L) return fail(NH_EINVAL, "null handle");
   if (n_lb < 0) return fail(NH_EINVAL, "n_lb must be >= 0");
   const int r = n_fd < 0 ? L->p.fd_ratio : n_fd;
-  NH_DISPATCH(L, (step_typed<double, true>(L, n_lb, r)), (step_typed<float, true>(L, n_lb, r)),
-              (step_typed<float, false>(L, n_lb, r)), (step_typed<double, false>(L, n_lb, r)));
+  if ((L->options & NH_OPT_GRAPH) && n_lb > 0) {
+    const int rc = step_graph(L, n_lb, r);
+    if (rc != NH_EAGAIN) return rc;          // the stream cannot be captured: plain launches
+  }
+  return step_plain(L, n_lb, r);
 }
 
 int nh_get_fields(nh_lattice* L, double* rho, double* u, double* n, double* F_lc) {
@@ -635,6 +700,7 @@ int nh_kernel_time(nh_lattice* L, int which, double* ms_total, long* launches) {
 void nh_free(nh_lattice* L) {
   if (!L) return;
   for (auto& pr : L->pool) { cudaEventDestroy(pr.a); cudaEventDestroy(pr.b); }
+  for (auto& g : L->graphs) cudaGraphExecDestroy(g.exec);
   delete L;
 }
 

@@ -196,11 +196,26 @@ def test_options_do_not_change_results():
         p = I.config(0, fd_ratio=3)
         d = p.pop("director")
         p.pop("steps")
-        g = m.Lattice(**dict(p, precision=0))
+        import torch
+        # graph replay needs a capturable stream (not the legacy default stream)
+        stream = torch.cuda.Stream() if opt & m.OPT_GRAPH else None
+        g = m.Lattice(stream=stream, **dict(p, precision=0))
         g.set_options(opt)
         g.set_director(d)
         g.step(50)
         g.step(31)
+        if opt & m.OPT_GRAPH:          # replays of cached graphs, and a schedule that cycles through keys
+            for _ in range(4):
+                g.step(3)
+            g.step(7)
+            h = m.Lattice(**dict(p, precision=0))
+            h.set_director(d)
+            h.step(100)
+            fg, fh = g.get_fields(), h.get_fields()
+            for k in fg:
+                assert np.array_equal(fg[k], fh[k]), k
+            assert g.launch_count == h.launch_count and g.time == h.time == 100
+            continue
         f = g.get_fields()
         if ref is None:
             ref = f
