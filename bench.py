@@ -40,7 +40,9 @@ def parse():
     ap.add_argument("--precision", default="fp32s", choices=sorted(PRECISIONS))
     ap.add_argument("--size", type=int, nargs=3, default=None, help="configs[4] grid (nx ny nz)")
     ap.add_argument("--options", type=lambda v: int(v, 0), default=0, help="nh_set_options bits (kernel variants)")
-    ap.add_argument("--two-step", action="store_true", help="NH_OPT_LB_TWOSTEP: two LB steps per launch through the L2")
+    ap.add_argument("--two-step", action="store_true", help="NH_OPT_LB_TWOSTEP: force two LB steps per launch through the L2")
+    ap.add_argument("--one-step", action="store_true", help="NH_OPT_LB_ONESTEP: one LB step per launch")
+    ap.add_argument("--block-order", action="store_true", help="NH_OPT_LB_BLOCKORDER: two-step units in blockIdx order")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -234,7 +236,8 @@ def main():
     lat = nh.Lattice(device="cuda:%d" % local, **dict(p, precision=prec))
     d_pinned = torch.from_numpy(d).pin_memory()
     lat.set_director(d_pinned)
-    base_opt = args.options | (nh.OPT_LB_TWOSTEP if args.two_step else 0)
+    base_opt = (args.options | (nh.OPT_LB_TWOSTEP if args.two_step else 0) | (nh.OPT_LB_ONESTEP if args.one_step else 0)
+                | (nh.OPT_LB_BLOCKORDER if args.block_order else 0))
 
     def barrier():
         torch.cuda.synchronize()

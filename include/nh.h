@@ -111,10 +111,15 @@ long nh_launch_count(const nh_lattice* L);
  *   bit4 NH_OPT_NO_SERPENTINE sweep the populations in the same direction on every launch
  *   bit5 NH_OPT_FD_NOVEC      stage the FD tiles element by element even where 16-byte copies fit
  *   bit6 NH_OPT_LB_TWOSTEP    two LB steps per launch through an L2-resident plane ring wherever no
- *                             director update falls between them (bit-identical results)
+ *                             director update falls between them and the grid tiles into pieces
+ *                             (nx a multiple of 64 that divides, or is a multiple of, 512);
+ *                             bit-identical results.  Without bit6 and bit7 the library decides
+ *                             (FP32, planes >= 256x256, ring <= 48 MB: DESIGN.md section 7).
+ *   bit7 NH_OPT_LB_ONESTEP    never use the two-step kernel
  *   bits 8-15                 planes per CTA of the tiled FD kernels (0 = chosen by the library)
  *   bits 16-19, 20-25         two-step kernel: lead D of phase 1 in planes, ring planes R (0 = default)
- *   bits 26-29                two-step kernel: persistent CTAs per SM (0 = occupancy limit)
+ *   bit26 NH_OPT_LB_BLOCKORDER two-step kernel: units in blockIdx order instead of by atomic ticket
+ *   bits 30, 31               two-step kernel: one cell per thread; 128-thread CTAs (tuning)
  * Setting options resets the timing accumulators. */
 #define NH_OPT_GRAPH          1
 #define NH_OPT_TIMING         2
@@ -123,6 +128,8 @@ long nh_launch_count(const nh_lattice* L);
 #define NH_OPT_NO_SERPENTINE 16
 #define NH_OPT_FD_NOVEC      32
 #define NH_OPT_LB_TWOSTEP    64
+#define NH_OPT_LB_ONESTEP   128
+#define NH_OPT_LB_BLOCKORDER (1 << 26)
 int nh_set_options(nh_lattice* L, int options);
 
 /* Accumulated CUDA-event time (ms) and number of launches of one kernel class since the last

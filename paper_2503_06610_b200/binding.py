@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(HERE, "libnh_b200.so")
 
 FP64_SHIFTED, FP32_SHIFTED, FP32_UNSHIFTED, FP64_UNSHIFTED = 0, 1, 2, 3
 OPT_GRAPH, OPT_TIMING, OPT_FD_DIRECT, OPT_LB_WIDE, OPT_NO_SERPENTINE, OPT_FD_NOVEC, OPT_LB_TWOSTEP = 1, 2, 4, 8, 16, 32, 64
+OPT_LB_ONESTEP, OPT_LB_BLOCKORDER = 128, 1 << 26
 KERNEL_CLASSES = ("lb", "velocity", "predictor", "corrector", "force", "other", "lb2")
 
 EXPORTS = ("nh_workspace_bytes", "nh_init_lattice", "nh_set_director", "nh_step", "nh_get_fields",

@@ -227,10 +227,26 @@ int lb2_cells_per_thread(const nh_lattice* L) {
   for (; U >= 1; --U) if (piece_grid(L, U, &g)) return U;
   return 0;
 }
+// Ring and lead of the wavefront (planes).  Defaults from the B200 measurements in DESIGN.md.
+void lb2_lead(const nh_lattice* L, int* D, int* R) {
+  *D = (L->options >> 16) & 0xf; *R = (L->options >> 20) & 0x3f;
+  if (*D == 0) *D = 4;
+  if (*R == 0) *R = *D + 4;
+  if (*R > L->ring_cap) *R = L->ring_cap;
+  if (*D > *R - 2) *D = *R - 2;
+}
 bool lb2_usable(const nh_lattice* L) {
   // (not under graph replay: a launch carries its own number and ticket base as arguments)
-  return (L->options & NH_OPT_LB_TWOSTEP) && !(L->options & NH_OPT_GRAPH) && L->ring_cap >= 3 &&
-         lb2_cells_per_thread(L) > 0;
+  if ((L->options & NH_OPT_LB_ONESTEP) || (L->options & NH_OPT_GRAPH) || L->ring_cap < 3) return false;
+  const int U = lb2_cells_per_thread(L);
+  if (U == 0) return false;
+  if (L->options & NH_OPT_LB_TWOSTEP) return true;
+  // automatic: only where it was measured to pay: FP32, a plane at least as
+  // large as the resident CTAs' work, and a ring that fits the L2 beside the streaming traffic
+  int D, R;
+  lb2_lead(L, &D, &R);
+  const double ring_mb = (double)R * 19.0 * L->G.plane * word_of(L->p.precision) / 1e6;
+  return word_of(L->p.precision) == 4 && L->G.plane >= 256u * 256u && ring_mb <= 48.0 && L->G.nz - 2 >= 4 * D;
 }
 
 template <typename T, bool SH, int U, int NT>
@@ -248,23 +264,14 @@ int launch_lb2_u(nh_lattice* L) {
   W.flag1 = (unsigned*)(L->wave + 8);
   W.flag2 = W.flag1 + (size_t)nzf * W.cps;
   W.nzf = nzf;
-  int D = (L->options >> 16) & 0xf, R = (L->options >> 20) & 0x3f;
-  if (D == 0) D = 5;
-  if (R == 0) R = D + 7;
-  if (R > L->ring_cap) R = L->ring_cap;
-  if (D > R - 2) D = R - 2;
+  int D, R;
+  lb2_lead(L, &D, &R);
   W.D = D; W.R = R;
   W.reverse = next_sweep(L);
   const unsigned long long units = 2ull * nzf * W.cps;
-  int per_sm_max = 0;
-  NH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_max, nh::lb_wave_kernel<T, SH, U, NT>, NT, 0));
-  int per_sm = ((L->options >> 26) & 0xf);
-  if (per_sm == 0 || per_sm > per_sm_max) per_sm = per_sm_max;
-  if (per_sm < 1) return fail(NH_ECUDA, "two-step LB kernel does not fit on an SM");
-  unsigned long long grid = (unsigned long long)per_sm * L->sm_count;
-  if (grid > units) grid = units;
+  if (L->options & NH_OPT_LB_BLOCKORDER) W.ticket = nullptr;
   W.ticket_base = L->wave_tickets;
-  L->wave_tickets += units + 3 * grid;      // every CTA draws three tickets past the end
+  if (W.ticket) L->wave_tickets += units;   // one ticket per CTA
   L->wave_epoch += 1;
   W.epoch = (unsigned)L->wave_epoch;
   nh::DirTab<const T> A;
@@ -274,7 +281,7 @@ int launch_lb2_u(nh_lattice* L) {
     B.p[i] = (T*)L->f[L->cur ^ 1] + (size_t)i * L->G.N;
     Rg.p[i] = (T*)L->ring + (size_t)i * R * L->G.plane;
   }
-  nh::lb_wave_kernel<T, SH, U, NT><<<(unsigned)grid, NT, 0, L->stream>>>(A, Rg, B, (const T*)L->F, L->G, lb_const<T>(L), W);
+  nh::lb_wave_kernel<T, SH, U, NT><<<(unsigned)units, NT, 0, L->stream>>>(A, Rg, B, (const T*)L->F, L->G, lb_const<T>(L), W);
   br.end();
   return NH_OK;
 }

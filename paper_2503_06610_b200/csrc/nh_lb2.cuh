@@ -12,19 +12,16 @@
 //
 // One launch runs both phases as a wavefront along z.
 //   Unit of work: one PIECE (256*U consecutive cells: whole rows, or a whole fraction of a row) of
-//   one plane of one phase.  Units are ordered -- phase 1 of planes 0..D, then phase 2 of plane k
-//   and phase 1 of plane k+D+1 alternating, piece by piece inside a plane -- and persistent CTAs
-//   draw them from an atomic ticket counter (the next ticket is fetched while the current unit is
-//   worked on).
+//   one plane of one phase, done by one CTA.  Units are ordered -- phase 1 of planes 0..D, then
+//   phase 2 of plane k and phase 1 of plane k+D+1 alternating, piece by piece inside a plane -- and
+//   a CTA takes the next unit from an atomic ticket counter when it starts to run.
 //   Dependencies are per-piece flags in global memory holding the launch number:
 //     phase 2 of (k, piece)  needs phase 1 of planes k-1, k, k+1 at the 3x3 neighbouring pieces
 //     phase 1 of (k, piece)  needs phase 2 of planes k-R-1 .. k-R+1 at the same pieces (the readers
 //                            of the ring slot it overwrites)
-//   Every unit depends only on units EARLIER in ticket order and a CTA holds at most one unfinished
-//   unit, so the earliest unfinished unit can always proceed: no deadlock, no cooperative launch.
-//   A wait longer than ~4 s sets an error flag instead of hanging the device.
-//   Per unit a CTA meets at ONE barrier (all stores issued; next ticket and its readiness known);
-//   thread 0 then publishes the unit with a store-release while the other warps go on.
+//   Every unit depends only on units EARLIER in ticket order, and a ticket is drawn by a CTA that
+//   is already running, so whatever a CTA waits for is running or done: no deadlock, no
+//   cooperative launch.  A wait longer than ~4 s sets an error flag instead of hanging the device.
 //
 // Each thread updates U cells 32 apart in x, so the address arithmetic is shared between them.
 // DRAM traffic per cell and PAIR of steps: 19 words read + 19 written (+ F^LC), against 2 x that
@@ -79,14 +76,6 @@ __device__ __forceinline__ void unit_of(unsigned m, int nzf, int D, int& phase, 
   phase = 2;
   k = pairs + (q - 2 * pairs);
 }
-
-// What a unit is, decoded once by thread 0 and handed to the CTA through shared memory.
-struct UnitInfo {
-  unsigned ticket;     // >= total: no more work
-  int phase, k;
-  unsigned prow, q;    // position in the piece grid
-  int ready;           // dependencies were seen complete by the prefetching warp
-};
 
 // 27 flags a unit depends on (3 planes x 3x3 pieces, periodic in the piece grid): lane l < 27
 // looks at one of them.  deps_look issues the acquire load and returns the flag (or "done" where
@@ -176,126 +165,99 @@ __device__ __forceinline__ void gather_cells(const Tab& S, unsigned zm, unsigned
 #undef NH_SHIFT
 }
 
-// Per unit a CTA meets at ONE barrier (all stores issued; the next unit and its readiness known);
-// thread 0 then publishes the unit with a store-release while the other warps go on.  Warp 0 looks
-// at the flags of the NEXT unit while its loads of the current one are in flight.
+// One CTA per unit.  The CTA draws its ticket when it starts to run (W.ticket != nullptr); with
+// NH_OPT_LB_BLOCKORDER the unit is blockIdx.x instead, which saves the atomic's round trip but relies
+// on CTAs being dispatched in blockIdx order (the hardware does, CUDA does not promise it; the
+// bounded waits turn a violation into an error flag, not a hang).  No loop-carried state; each warp
+// checks the flags itself (27 lanes, one acquire load).  A phase-1 unit gathers first and checks
+// its flags (the old readers of its ring slot) only before it stores; a phase-2 unit checks before
+// it gathers.  One barrier at the end, then thread 0 publishes the unit with a store-release.
 template <typename T, bool SHIFTED, int U, int NT>
-__global__ void __launch_bounds__(NT, (sizeof(T) == 4 ? (U == 2 ? 3 : 4) : (U == 2 ? 1 : 2)) * (256 / NT))
+__global__ void __launch_bounds__(NT, (sizeof(T) == 4 ? 4 : (U == 2 ? 1 : 2)) * (256 / NT))
 lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restrict__ Flc,
-               Geom G, LbConst<T> C, Wave W) {
-  __shared__ UnitInfo s_info[3];
+                Geom G, LbConst<T> C, Wave W) {
   const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-  const unsigned total = 2u * (unsigned)W.nzf * W.cps;
-
-  auto decode = [&](unsigned tk, UnitInfo& I) {
-    I.ticket = tk;
-    I.ready = 0;
-    if (tk < total) {
-      const unsigned unit = tk / W.cps, piece = tk - unit * W.cps;
-      unit_of(unit, W.nzf, W.D, I.phase, I.k);
-      I.prow = piece / W.ppr;
-      I.q = piece - I.prow * W.ppr;
+  unsigned tk = blockIdx.x;
+  if (W.ticket) {                       // safe order: a ticket drawn when the CTA starts to run
+    __shared__ unsigned s_tk;
+    if (threadIdx.x == 0) s_tk = (unsigned)(atomicAdd(W.ticket, 1ull) - W.ticket_base);
+    __syncthreads();
+    tk = s_tk;
+  }
+  const unsigned unit = tk / W.cps, piece = tk - unit * W.cps;
+  int phase, k;
+  unit_of(unit, W.nzf, W.D, phase, k);
+  const unsigned prow = piece / W.ppr, q = piece - prow * W.ppr;
+  auto wait_flags = [&]() {
+    const long long t0 = clock64();
+    unsigned ns = 32;
+    while (!deps_ready(W, phase, k, prow, q, lane)) {
+      __nanosleep(ns);
+      if (ns < 512) ns *= 2;
+      if (clock64() - t0 > 8000000000ll) { if (lane == 0) atomicExch(W.err, 1); break; }
     }
   };
-  // thread 0 keeps three tickets ahead: this unit and the next are decoded in shared memory when
-  // a unit starts (so the next one can be warmed and looked at), the one after that is decoded
-  // while this one is worked on, and a fourth ticket is in flight
-  unsigned long long tnext = 0;
-  if (threadIdx.x == 0) {
-    decode((unsigned)(atomicAdd(W.ticket, 1ull) - W.ticket_base), s_info[0]);
-    decode((unsigned)(atomicAdd(W.ticket, 1ull) - W.ticket_base), s_info[1]);
-    tnext = atomicAdd(W.ticket, 1ull);
+  const unsigned seg_row = warp >> W.spr_shift;
+  const unsigned seg_x = (warp & ((1u << W.spr_shift) - 1u)) * (32u * U);
+  const int z = (W.reverse ? W.nzf - 1 - k : k) + 1;
+  const unsigned y = prow * W.rows_per_piece + seg_row;
+  const unsigned xA = q * (unsigned)(NT * U) + seg_x + lane;
+  const bool active = y < (unsigned)G.ny;
+  const unsigned nx = (unsigned)G.nx;
+  const unsigned r0 = y * nx;
+  const unsigned slot = (unsigned)((z - 1) % W.R);
+  const unsigned cell = (unsigned)z * G.plane + r0 + xA;
+  if (phase == 2) wait_flags();
+  Pop<T> P[U];
+  T Fx[U], Fy[U], Fz[U];
+  if (active) {
+    const unsigned rm = (y == 0 ? (unsigned)G.ny - 1 : y - 1) * nx;
+    const unsigned rp = (y == (unsigned)G.ny - 1 ? 0u : y + 1) * nx;
+    const bool lo = (z == 1), hi = (z == G.nz - 2);
+    if (phase == 1) {
+      const unsigned z0 = (unsigned)z * G.plane;
+      gather_cells<T, LD_CS, U>(A, z0 - G.plane, z0, z0 + G.plane, r0, rm, rp, xA, nx, lo, hi, P);
+    } else {
+      const unsigned sm = (slot == 0 ? (unsigned)W.R - 1 : slot - 1), sp = (slot == (unsigned)W.R - 1 ? 0u : slot + 1);
+      gather_cells<T, LD_CG, U>(ring, sm * G.plane, slot * G.plane, sp * G.plane, r0, rm, rp, xA, nx, lo, hi, P);
+    }
+#pragma unroll
+    for (int j = 0; j < U; ++j) {
+      Fx[j] = Fy[j] = Fz[j] = T(0);
+      if (C.use_flc) {
+        const T* f = Flc + cell;
+        Fx[j] = __ldg(f + 32 * j); Fy[j] = __ldg(f + G.N + 32 * j); Fz[j] = __ldg(f + 2 * G.N + 32 * j);
+      }
+    }
+  }
+  unsigned look = 0xffffffffu;
+  if (phase == 1) look = deps_look(W, phase, k, prow, q, lane);
+  if (active) {
+#pragma unroll
+    for (int j = 0; j < U; ++j) collide<T, SHIFTED>(P[j], Fx[j], Fy[j], Fz[j], C);
+  }
+  if (phase == 1 && !deps_test(W, look)) wait_flags();
+  if (active) {
+    if (phase == 1) {
+      const unsigned o = slot * G.plane + r0 + xA;
+#pragma unroll
+      for (int i = 0; i < Q; ++i) {
+        T* d = ring.p[i] + o;
+#pragma unroll
+        for (int j = 0; j < U; ++j) d[32 * j] = P[j].f[i];
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < Q; ++i) {
+        T* d = B.p[i] + cell;
+#pragma unroll
+        for (int j = 0; j < U; ++j) __stcs(d + 32 * j, P[j].f[i]);
+      }
+    }
   }
   __syncthreads();
-
-  // this thread's place inside a piece
-  const unsigned seg_row = warp >> W.spr_shift;                             // lattice row inside the piece
-  const unsigned seg_x = (warp & ((1u << W.spr_shift) - 1u)) * (32u * U);   // first column of the warp's segment
-  unsigned b0 = 0;
-  for (;;) {
-    const unsigned b1 = (b0 == 2 ? 0u : b0 + 1), b2 = (b1 == 2 ? 0u : b1 + 1);
-    const UnitInfo I = s_info[b0];
-    if (I.ticket >= total) break;
-    const UnitInfo Nx = s_info[b1];
-    if (threadIdx.x == 0) {
-      decode((unsigned)(tnext - W.ticket_base), s_info[b2]);
-      tnext = atomicAdd(W.ticket, 1ull);                        // consumed one unit later
-    }
-    if (!I.ready) {
-      const long long t0 = clock64();
-      unsigned ns = 32;
-      while (!deps_ready(W, I.phase, I.k, I.prow, I.q, lane)) {
-        __nanosleep(ns);
-        if (ns < 512) ns *= 2;
-        if (clock64() - t0 > 8000000000ll) { if (lane == 0) atomicExch(W.err, 1); break; }
-      }
-    }
-
-    const int z = (W.reverse ? W.nzf - 1 - I.k : I.k) + 1;                  // physical plane
-    const unsigned y = I.prow * W.rows_per_piece + seg_row;
-    const unsigned xA = I.q * (unsigned)(NT * U) + seg_x + lane;
-    const bool active = y < (unsigned)G.ny;
-    const unsigned nx = (unsigned)G.nx;
-    const unsigned r0 = y * nx;
-    const unsigned slot = (unsigned)((z - 1) % W.R);
-    const unsigned cell = (unsigned)z * G.plane + r0 + xA;
-    Pop<T> P[U];
-    T Fx[U], Fy[U], Fz[U];
-    if (active) {
-      const unsigned rm = (y == 0 ? (unsigned)G.ny - 1 : y - 1) * nx;
-      const unsigned rp = (y == (unsigned)G.ny - 1 ? 0u : y + 1) * nx;
-      const bool lo = (z == 1), hi = (z == G.nz - 2);
-      if (I.phase == 1) {
-        const unsigned z0 = (unsigned)z * G.plane;
-        gather_cells<T, LD_CS, U>(A, z0 - G.plane, z0, z0 + G.plane, r0, rm, rp, xA, nx, lo, hi, P);
-      } else {
-        const unsigned sm = (slot == 0 ? (unsigned)W.R - 1 : slot - 1), sp = (slot == (unsigned)W.R - 1 ? 0u : slot + 1);
-        gather_cells<T, LD_CG, U>(ring, sm * G.plane, slot * G.plane, sp * G.plane, r0, rm, rp, xA, nx, lo, hi, P);
-      }
-#pragma unroll
-      for (int j = 0; j < U; ++j) {
-        Fx[j] = Fy[j] = Fz[j] = T(0);
-        if (C.use_flc) {
-          const T* f = Flc + cell;
-          Fx[j] = __ldg(f + 32 * j); Fy[j] = __ldg(f + G.N + 32 * j); Fz[j] = __ldg(f + 2 * G.N + 32 * j);
-        }
-      }
-    }
-    // warp 0: a look (not a wait: this unit is not published yet) at the flags of the next unit; the
-    // answer is needed only after this unit's stores, so its latency hides under the work
-    unsigned look = 0;
-    if (warp == 0 && Nx.ticket < total) look = deps_look(W, Nx.phase, Nx.k, Nx.prow, Nx.q, lane);
-    if (active) {
-#pragma unroll
-      for (int j = 0; j < U; ++j) collide<T, SHIFTED>(P[j], Fx[j], Fy[j], Fz[j], C);
-      if (I.phase == 1) {
-        const unsigned o = slot * G.plane + r0 + xA;
-#pragma unroll
-        for (int i = 0; i < Q; ++i) {
-          T* d = ring.p[i] + o;
-#pragma unroll
-          for (int j = 0; j < U; ++j) d[32 * j] = P[j].f[i];
-        }
-      } else {
-#pragma unroll
-        for (int i = 0; i < Q; ++i) {
-          T* d = B.p[i] + cell;
-#pragma unroll
-          for (int j = 0; j < U; ++j) __stcs(d + 32 * j, P[j].f[i]);
-        }
-      }
-    }
-    if (warp == 0) {
-      const bool ok = deps_test(W, look);
-      if (lane == 0) s_info[b1].ready = (ok && Nx.ticket < total) ? 1 : 0;
-    }
-    __syncthreads();      // every store of this unit is issued; s_info[b1], s_info[b2] are complete
-    if (threadIdx.x == 0) {
-      unsigned* f = (I.phase == 1 ? W.flag1 : W.flag2) + (size_t)I.k * W.cps + I.prow * W.ppr + I.q;
-      st_release_u32(f, W.epoch);
-    }
-    b0 = b1;
-  }
+  if (threadIdx.x == 0)
+    st_release_u32((phase == 1 ? W.flag1 : W.flag2) + (size_t)k * W.cps + prow * W.ppr + q, W.epoch);
 }
 
 }  // namespace nh

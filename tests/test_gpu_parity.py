@@ -252,9 +252,9 @@ def test_two_step_kernel_is_bit_identical(shape, r):
 
     T = m.OPT_LB_TWOSTEP
     for precision in (0, 1):
-        ref = run(precision, 0, [43])
+        ref = run(precision, m.OPT_LB_ONESTEP, [43])
         for opt in (T, T | m.OPT_NO_SERPENTINE, T | (1 << 30), T | (1 << 31), T | (1 << 16) | (3 << 20),
-                    T | (3 << 16) | (12 << 20) | (2 << 26)):
+                    T | (3 << 16) | (12 << 20) | m.OPT_LB_BLOCKORDER, T | m.OPT_LB_BLOCKORDER | (1 << 30)):
             f = run(precision, opt, [1, 7, 20, 15])
             for k in ref:
                 assert np.array_equal(ref[k], f[k]), (shape, precision, hex(opt), k)
@@ -262,10 +262,10 @@ def test_two_step_kernel_is_bit_identical(shape, r):
 
 def test_config3_full_size_bench_configuration():
     """BASELINE.json configs[3] at FULL size (256x256x64, two tubes, r = 10), in the launch
-    configurations bench.py times (default options, and the two-step LB kernel): FP64 within 1e-10
-    at 100 steps, shifted FP32 within (1e-3, 1e-4) at 100 and at 1000 steps (north_star's bar), every
-    output element compared with the oracle; the two-step run must equal the default FP32 run bit
-    for bit.  One oracle run (about 90 s of host time) serves all of them."""
+    configurations bench.py times (default options: the two-step LB kernel in FP32; and one step
+    per launch): FP64 within 1e-10 at 100 steps, shifted FP32 within (1e-3, 1e-4) at 100 and at 1000
+    steps (north_star's bar), every output element compared with the oracle; the one-step run must
+    equal the default FP32 run bit for bit.  One oracle run (about 90 s of host time) serves all of them."""
     m = nh()
     p = I.config(3)
     d = p.pop("director")
@@ -275,7 +275,7 @@ def test_config3_full_size_bench_configuration():
     g64 = m.Lattice(**dict(p, precision=0))
     g32 = m.Lattice(**dict(p, precision=1))
     g32w = m.Lattice(**dict(p, precision=1))
-    g32w.set_options(m.OPT_LB_TWOSTEP)
+    g32w.set_options(m.OPT_LB_ONESTEP)
     for g in (g64, g32, g32w):
         g.set_director(d)
     for n in (100, 900):
@@ -288,7 +288,8 @@ def test_config3_full_size_bench_configuration():
         a, b = g32.get_fields(), g32w.get_fields()
         for k in a:
             assert np.array_equal(a[k], b[k]), k
-    assert g32w.kernel_time("lb2")[1] > 0 and g32.kernel_time("lb2")[1] == 0
+    # the default picks the two-step kernel on this grid in FP32 and the one-step kernel in FP64
+    assert g32.kernel_time("lb2")[1] > 0 and g32w.kernel_time("lb2")[1] == 0 and g64.kernel_time("lb2")[1] == 0
     f = g64.get_fields()
     nf = p["nx"] * p["ny"] * (p["nz"] - 2)
     assert abs((f["rho"][1:-1] - 1.0).sum()) / nf < 1e-12          # mass (pin P2) on the GPU at full size
