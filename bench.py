@@ -112,7 +112,7 @@ class ClockSampler:
     def stop(self):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.06)
+        time.sleep(0.25)          # nvidia-smi -lms needs a moment to print its first line on short runs
         self.proc.terminate()
         try:
             out = self.proc.communicate(timeout=5)[0]
@@ -295,6 +295,14 @@ def main():
                 "full_step_bytes_per_cell": (41 + 30.0 / r) * word,
                 "full_step_achieved_gbs": (41 + 30.0 / r) * word * nf * r * args.steps / (ms * 1e-3) / 1e9,
                 "timed": "second pass of the same K steps with per-launch CUDA events on the launch stream"}
+    if roofline["traffic"] and lb_avg > 0:
+        # what the DRAM actually moved (ncu capture of the same kernel) over the live launch time
+        roofline["dram_gbs"] = roofline["traffic"] / (lb_avg * 1e-3) / 1e9
+        roofline["dram_frac"] = roofline["dram_gbs"] / peak
+    if two:
+        roofline["note"] = ("two LB steps share one pass over HBM (the intermediate step lives in an L2-resident "
+                            "plane ring), so the algorithmic bytes of two steps move in about the DRAM traffic of "
+                            "one: frac > 1 is expected; dram_frac is the DRAM's own utilisation")
 
     # ---- end to end through the C ABI with host buffers --------------------------------------------
     e2e = None

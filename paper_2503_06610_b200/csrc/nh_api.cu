@@ -64,7 +64,7 @@ int ring_planes(const nh_params* p) { return p->nz - 2 < 12 ? p->nz - 2 : 12; }
 // u64 words of the two-step kernel's control block: 8 header words, then two u32 flags per plane and piece
 size_t wave_words(const nh_params* p) {
   const size_t pieces = (size_t)p->nx * p->ny / 128 + p->ny + 1;   // upper bound over the piece shapes
-  return 8 + (size_t)(p->nz - 2) * pieces;
+  return 8 + (size_t)(p->nz - 2) * pieces + (size_t)(p->nz - 2) + 8;   // + the launch-order table
 }
 
 }  // namespace
@@ -93,6 +93,9 @@ struct nh_lattice {
   int ring_cap;     // planes it holds
   unsigned long long* wave;   // device counters of the two-step kernel: err flag at [4], done1, done2 from [8]
   unsigned long long wave_epoch, wave_tickets;
+  unsigned* order_dev;             // launch order table of the two-step kernel
+  unsigned order_len;
+  int order_key;                   // (D << 8) | nzf the tables were built for, -1: none
   int sm_count;
   // CUDA-graph replay of nh_step (NH_OPT_GRAPH): one executable graph per distinct call shape
   struct Graph {
@@ -249,6 +252,27 @@ bool lb2_usable(const nh_lattice* L) {
   return word_of(L->p.precision) == 4 && L->G.plane >= 256u * 256u && ring_mb <= 48.0 && L->G.nz - 2 >= 4 * D;
 }
 
+// Launch order of the wavefront: round j emits phase 2 of plane j-D-1, then phase 1 of plane j --
+// every unit after everything it waits for.
+int lb2_order(nh_lattice* L, int D) {
+  const int nzf = L->G.nz - 2;
+  const int key = (D << 16) | nzf;
+  if (L->order_key == key) return NH_OK;
+  const size_t pieces = (size_t)L->G.nx * L->G.ny / 128 + L->G.ny + 1;
+  std::vector<unsigned> o;
+  for (int j = 0; j < nzf + D + 1; ++j) {
+    const int k2 = j - D - 1;
+    if (k2 >= 0 && k2 < nzf) o.push_back((2u << 16) | (unsigned)k2);
+    if (j < nzf) o.push_back((1u << 16) | (unsigned)j);
+  }
+  L->order_dev = (unsigned*)(L->wave + 8 + (size_t)nzf * pieces);
+  L->order_len = (unsigned)o.size();
+  NH_CUDA(cudaMemcpyAsync(L->order_dev, o.data(), o.size() * sizeof(unsigned), cudaMemcpyHostToDevice, L->stream));
+  NH_CUDA(cudaStreamSynchronize(L->stream));     // o goes out of scope
+  L->order_key = key;
+  return NH_OK;
+}
+
 template <typename T, bool SH, int U, int NT>
 int launch_lb2_u(nh_lattice* L) {
   Bracket br(L, KC_LB2);
@@ -267,8 +291,10 @@ int launch_lb2_u(nh_lattice* L) {
   int D, R;
   lb2_lead(L, &D, &R);
   W.D = D; W.R = R;
+  { const int rc = lb2_order(L, D); if (rc) return rc; }
+  W.order = L->order_dev;
   W.reverse = next_sweep(L);
-  const unsigned long long units = 2ull * nzf * W.cps;
+  const unsigned long long units = (unsigned long long)L->order_len * W.cps;
   if (L->options & NH_OPT_LB_BLOCKORDER) W.ticket = nullptr;
   W.ticket_base = L->wave_tickets;
   if (W.ticket) L->wave_tickets += units;   // one ticket per CTA
@@ -627,7 +653,7 @@ int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_strea
   L->ring_cap = ring_planes(p);
   L->ring = take((size_t)L->ring_cap * 19 * L->G.plane * w);
   L->wave = (unsigned long long*)take(wave_words(p) * 8);
-  L->wave_epoch = 0; L->wave_tickets = 0;
+  L->wave_epoch = 0; L->wave_tickets = 0; L->order_key = -1;
   e = cudaMemsetAsync(L->wave, 0, wave_words(p) * 8, L->stream);
   if (e != cudaSuccess) { delete L; return cuda_fail(e, "cudaMemsetAsync(wave)"); }
   int rc;

@@ -48,6 +48,7 @@ struct Wave {
   int D;                          // lead of phase 1 over phase 2, in planes (>= 1)
   int R;                          // ring slots (planes), R >= D + 2
   int reverse;                    // sweep from the top plate down
+  const unsigned* order;          // [units per launch] (phase << 16) | logical plane, in launch order
 };
 
 // p[i] = start of direction i inside a population array
@@ -62,21 +63,6 @@ __device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
   asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// Unit m of the launch order -> (phase, logical plane k).
-__device__ __forceinline__ void unit_of(unsigned m, int nzf, int D, int& phase, int& k) {
-  const int lead = min(D + 1, nzf);            // phase-1 planes before the first phase-2 plane
-  if ((int)m < lead) { phase = 1; k = (int)m; return; }
-  const int q = (int)m - lead;
-  const int pairs = nzf - lead;                // phase-1 planes left to interleave
-  if (q < 2 * pairs) {
-    if (q & 1) { phase = 1; k = lead + (q >> 1); }
-    else       { phase = 2; k = q >> 1; }
-    return;
-  }
-  phase = 2;
-  k = pairs + (q - 2 * pairs);
-}
-
 // 27 flags a unit depends on (3 planes x 3x3 pieces, periodic in the piece grid): lane l < 27
 // looks at one of them.  deps_look issues the acquire load and returns the flag (or "done" where
 // there is nothing to wait for); deps_test is the vote over the warp.
@@ -87,8 +73,11 @@ __device__ __forceinline__ unsigned deps_look(const Wave& W, int phase, int k, u
     const int j = (phase == 2 ? k - 1 : k - W.R - 1) + (int)(lane / 9);
     if (j >= 0 && j < W.nzf) {
       const unsigned r9 = lane % 9, dr = r9 / 3, dq = r9 % 3;      // 0, 1, 2 -> -1, 0, +1
-      const unsigned pr = (prow + W.prows + dr - 1) % W.prows;
-      const unsigned pq = (q + W.ppr + dq - 1) % W.ppr;
+      unsigned pr = prow + dr, pq = q + dq;                        // periodic wrap without a division
+      pr = (pr == 0) ? W.prows - 1 : pr - 1;
+      if (pr == W.prows) pr = 0;
+      pq = (pq == 0) ? W.ppr - 1 : pq - 1;
+      if (pq == W.ppr) pq = 0;
       v = ld_acquire_u32((phase == 2 ? W.flag1 : W.flag2) + (size_t)j * W.cps + pr * W.ppr + pq);
     }
   }
@@ -175,19 +164,28 @@ __device__ __forceinline__ void gather_cells(const Tab& S, unsigned zm, unsigned
 template <typename T, bool SHIFTED, int U, int NT>
 __global__ void __launch_bounds__(NT, (sizeof(T) == 4 ? 4 : (U == 2 ? 1 : 2)) * (256 / NT))
 lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restrict__ Flc,
-                Geom G, LbConst<T> C, Wave W) {
+               Geom G, LbConst<T> C, Wave W) {
   const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-  unsigned tk = blockIdx.x;
-  if (W.ticket) {                       // safe order: a ticket drawn when the CTA starts to run
-    __shared__ unsigned s_tk;
-    if (threadIdx.x == 0) s_tk = (unsigned)(atomicAdd(W.ticket, 1ull) - W.ticket_base);
-    __syncthreads();
-    tk = s_tk;
-  }
-  const unsigned unit = tk / W.cps, piece = tk - unit * W.cps;
+  // which unit: decoded once (by thread 0 from its ticket, or by everyone from blockIdx, which the
+  // compiler keeps on the uniform datapath)
   int phase, k;
-  unit_of(unit, W.nzf, W.D, phase, k);
-  const unsigned prow = piece / W.ppr, q = piece - prow * W.ppr;
+  unsigned prow, q;
+  if (W.ticket) {                       // safe order: a ticket drawn when the CTA starts to run
+    __shared__ int s_unit[4];
+    if (threadIdx.x == 0) {
+      const unsigned tk = (unsigned)(atomicAdd(W.ticket, 1ull) - W.ticket_base);
+      const unsigned unit = tk / W.cps, piece = tk - unit * W.cps;
+      const unsigned code = W.order[unit];
+      s_unit[0] = (int)(code >> 16); s_unit[1] = (int)(code & 0xffffu); s_unit[2] = (int)(piece / W.ppr); s_unit[3] = (int)(piece % W.ppr);
+    }
+    __syncthreads();
+    phase = s_unit[0]; k = s_unit[1]; prow = (unsigned)s_unit[2]; q = (unsigned)s_unit[3];
+  } else {
+    const unsigned unit = blockIdx.x / W.cps, piece = blockIdx.x - unit * W.cps;
+    const unsigned code = W.order[unit];
+    phase = (int)(code >> 16); k = (int)(code & 0xffffu);
+    prow = piece / W.ppr; q = piece - prow * W.ppr;
+  }
   auto wait_flags = [&]() {
     const long long t0 = clock64();
     unsigned ns = 32;
