@@ -187,6 +187,83 @@ void elastic_force_field(const Grid& G, double K, double q0, const double* n, do
         }
 }
 
+// Leslie viscous stress, Eq. 3 as it enters the force of Eq. 12, with
+// alpha_4 replaced by alpha_4':
+//   sigma^v_ab = a1 n_a n_b n_m n_r D_mr + a2 n_b N_a + a3 n_a N_b + a4' D_ab + a5 n_b n_m D_ma + a6 n_a n_m D_mb
+// al[] = {alpha1, alpha2, alpha3, alpha4', alpha5, alpha6}.  D as printed in Eq. 5.  The co-rotational
+// rate N of Eq. 4 is taken from Eq. 9: N = d_t n + (u.grad) n - W.n = h/gamma1 + xi n.D, projected
+// perpendicular to n like the director's rate itself (reading G22), so no time derivative
+// is needed.
+void viscous_stress_cell(const Grid& G, double K, double q0, double xi, double gamma1, const double al[6],
+                         const double* n, const double* u, int x, int y, int z, double sig[3][3]) {
+  const size_t N = G.N();
+  const size_t c0 = G.at(x, y, z);
+  double du[3][3];  // d_b u_c
+  for (int b = 0; b < 3; ++b)
+    for (int c = 0; c < 3; ++c) du[b][c] = ddx(G, u, c, x, y, z, b);
+  double D[3][3];
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b) D[a][b] = 0.5 * (du[a][b] + du[b][a]);
+  const double nn[3] = {n[c0], n[N + c0], n[2 * N + c0]};
+  double h[3];
+  molecular_field_cell(G, K, q0, n, x, y, z, h);
+  double nD[3], A[3];  // nD_b = n_m D_mb
+  for (int b = 0; b < 3; ++b) {
+    nD[b] = 0.0;
+    for (int m = 0; m < 3; ++m) nD[b] += nn[m] * D[m][b];
+    A[b] = h[b] / gamma1 + xi * nD[b];
+  }
+  const double nA = nn[0] * A[0] + nn[1] * A[1] + nn[2] * A[2];
+  double Nr[3];
+  for (int b = 0; b < 3; ++b) Nr[b] = A[b] - nA * nn[b];
+  double nnD = 0.0;  // n_m n_r D_mr
+  for (int m = 0; m < 3; ++m) nnD += nn[m] * nD[m];
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b)
+      sig[a][b] = al[0] * nn[a] * nn[b] * nnD + al[1] * nn[b] * Nr[a] + al[2] * nn[a] * Nr[b] +
+                  al[3] * D[a][b] + al[4] * nn[b] * nD[a] + al[5] * nn[a] * nD[b];
+}
+
+bool any_alpha(const double al[6]) {
+  for (int i = 0; i < 6; ++i)
+    if (al[i] != 0.0) return true;
+  return false;
+}
+
+// sigma (+)= sigma^v on the computed layers; the plate layers stay 0 (G6).
+void viscous_stress_add(const Grid& G, double K, double q0, double xi, double gamma1, const double al[6],
+                        const double* n, const double* u, double* sigma) {
+  const size_t N = G.N();
+#pragma omp parallel for schedule(static)
+  for (int z = G.z_lo(); z < G.z_hi(); ++z)
+    for (int y = 0; y < G.ny; ++y)
+      for (int x = 0; x < G.nx; ++x) {
+        double s[3][3];
+        viscous_stress_cell(G, K, q0, xi, gamma1, al, n, u, x, y, z, s);
+        for (int a = 0; a < 3; ++a)
+          for (int b = 0; b < 3; ++b) sigma[(3 * a + b) * N + G.at(x, y, z)] += s[a][b];
+      }
+}
+
+// F^LC_a = d_b (sigma^e_ab + sigma^v_ab) by central differences: Eq. 12.
+void lc_force_field(const Grid& G, double K, double q0, double xi, double gamma1, const double al[6],
+                    const double* n, const double* u, double* F, std::vector<double>& sigma) {
+  const size_t N = G.N();
+  sigma.resize(9 * N);
+  elastic_stress_field(G, K, q0, n, sigma.data());
+  if (any_alpha(al)) viscous_stress_add(G, K, q0, xi, gamma1, al, n, u, sigma.data());
+  std::memset(F, 0, sizeof(double) * 3 * N);
+#pragma omp parallel for schedule(static)
+  for (int z = G.z_lo(); z < G.z_hi(); ++z)
+    for (int y = 0; y < G.ny; ++y)
+      for (int x = 0; x < G.nx; ++x)
+        for (int a = 0; a < 3; ++a) {
+          double s = 0.0;
+          for (int b = 0; b < 3; ++b) s += ddx(G, sigma.data(), 3 * a + b, x, y, z, b);
+          F[a * N + G.at(x, y, z)] = s;
+        }
+}
+
 void director_rhs_field(const Grid& G, double K, double q0, double xi, double gamma1,
                         const double* m, const double* u, double* R) {
   const size_t N = G.N();
@@ -213,7 +290,7 @@ struct nh_oracle_lattice {
   long t;
   std::vector<double> f, fnew;            // populations [i][cell]: f^shifted (Eq. 19) or f
   std::vector<double> n, nP, nnew, u, F;  // director, predictor, velocity scratch, F^LC
-  std::vector<double> k1, k2, sigma;
+  std::vector<double> k1, k2, sigma, uv;  // uv: u(t) for the viscous stress (whatever coupling bit1 says)
 
   // Moments of one fluid cell.  Shifted: Eqs. 20-21; unshifted: Eqs. 16-17
   // (PAPER.md:131-135).  Ftot = [coupling bit0] F^LC + rho g (reading G8).
@@ -313,6 +390,15 @@ struct nh_oracle_lattice {
         }
   }
 
+  // F^LC from the current director (and, for the viscous part, the current velocity).
+  void lc_force(bool have_u) {
+    const double* uu = u.data();
+    if (any_alpha(p.alpha)) {
+      if (!have_u) { uv.resize(3 * G.N()); velocity_field(nullptr, uv.data()); uu = uv.data(); }
+    }
+    lc_force_field(G, p.K, q0, p.xi, p.gamma1, p.alpha, n.data(), uu, F.data(), sigma);
+  }
+
   // FD update with Delta t_FD = r, same u for both stages (G11).
   void fd_update(int r) {
     const size_t N = G.N();
@@ -324,7 +410,7 @@ struct nh_oracle_lattice {
     director_rhs_field(G, p.K, q0, p.xi, p.gamma1, nP.data(), u.data(), k2.data());  // (d_t n)_P
     normalise_into(nnew, n, k1, &k2, dt);                                            // corrector
     n.swap(nnew);
-    elastic_force_field(G, p.K, q0, n.data(), F.data(), sigma);                      // Eq. 12
+    lc_force(/*have_u=*/(p.coupling & 2) != 0);                                     // Eq. 12
     (void)N;
   }
 };
@@ -410,7 +496,7 @@ int nh_oracle_set_director(nh_oracle_lattice* L, const double* n_host) {
       }
   }
   L->nP = L->n;
-  elastic_force_field(L->G, L->p.K, L->q0, L->n.data(), L->F.data(), L->sigma);  // reading G9
+  L->lc_force(/*have_u=*/false);  // reading G9
   return 0;
 }
 
@@ -502,6 +588,25 @@ int nh_oracle_elastic_force(int nx, int ny, int nz, int periodic_z, double K, do
   const Grid G{nx, ny, nz, periodic_z != 0};
   std::vector<double> sigma;
   elastic_force_field(G, K, q0, n, F, sigma);
+  return 0;
+}
+
+int nh_oracle_viscous_stress(int nx, int ny, int nz, int periodic_z, double K, double q0, double xi,
+                             double gamma1, const double* alpha, const double* n, const double* u,
+                             double* sigma) {
+  if (!n || !u || !sigma || !alpha || bad_dims(nx, ny, nz) || !(gamma1 > 0.0)) return fail(E_INVAL, "bad arguments");
+  const Grid G{nx, ny, nz, periodic_z != 0};
+  std::memset(sigma, 0, sizeof(double) * 9 * G.N());
+  viscous_stress_add(G, K, q0, xi, gamma1, alpha, n, u, sigma);
+  return 0;
+}
+
+int nh_oracle_lc_force(int nx, int ny, int nz, int periodic_z, double K, double q0, double xi,
+                       double gamma1, const double* alpha, const double* n, const double* u, double* F) {
+  if (!n || !u || !F || !alpha || bad_dims(nx, ny, nz) || !(gamma1 > 0.0)) return fail(E_INVAL, "bad arguments");
+  const Grid G{nx, ny, nz, periodic_z != 0};
+  std::vector<double> sigma;
+  lc_force_field(G, K, q0, xi, gamma1, alpha, n, u, F, sigma);
   return 0;
 }
 

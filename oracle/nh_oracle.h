@@ -13,7 +13,8 @@
  *   FD   : central differences Eq. 13, solid values fixed,
  *          director equation Eq. 9 with D, W of Eq. 5,
  *          predictor-corrector PAPER.md:105-112
- *   force: Eq. 6 and the last term of Eq. 12
+ *   force: Eq. 6 and the last term of Eq. 12; optionally the Leslie
+ *          viscous stress of Eq. 3 in Eq. 12 (row f1, pins V1-V4)
  *   loop : Fig. 1 / Sec. II.D
  * Readings of gaps in the paper are SURVEY.md Sec. 8(c) G1-G21, listed in DESIGN.md.
  *
@@ -53,6 +54,9 @@ typedef struct {
   int    precision;    /* 0,1: shifted populations (Eqs. 19-23); 2,3: unshifted (Eqs. 14-17).
                           The oracle computes in FP64 whatever this says.                  */
   int    coupling;     /* bit0: F^LC acts on the flow; bit1: flow acts on n               */
+  double alpha[6];     /* Leslie viscosities alpha1, alpha2, alpha3, alpha4', alpha5, alpha6 of the
+                          viscous stress in the force, Eqs. 3, 12; all 0 = elastic stress only
+                                                                         PAPER.md:50, 97-99 */
 } nh_oracle_params;
 
 int  nh_oracle_init_lattice(const nh_oracle_params*, nh_oracle_lattice** out);
@@ -79,6 +83,13 @@ int nh_oracle_elastic_stress(int nx, int ny, int nz, int periodic_z, double K, d
                              const double* n, double* sigma /* [9][nz][ny][nx], index 3*alpha+beta */);
 int nh_oracle_elastic_force(int nx, int ny, int nz, int periodic_z, double K, double q0,
                             const double* n, double* F);
+/* Leslie viscous stress of Eq. 3 with alpha4 -> alpha4' (Eq. 12), N from Eq. 9 (reading G22), and
+ * the whole force F^LC = d_b (sigma^e + sigma^v)_ab.  alpha = {a1, a2, a3, a4', a5, a6}. */
+int nh_oracle_viscous_stress(int nx, int ny, int nz, int periodic_z, double K, double q0, double xi,
+                             double gamma1, const double* alpha, const double* n, const double* u,
+                             double* sigma /* [9][nz][ny][nx] */);
+int nh_oracle_lc_force(int nx, int ny, int nz, int periodic_z, double K, double q0, double xi,
+                       double gamma1, const double* alpha, const double* n, const double* u, double* F);
 
 #ifdef __cplusplus
 }

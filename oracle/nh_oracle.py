@@ -12,7 +12,7 @@ class _Params(C.Structure):
                 ("tau", C.c_double), ("K", C.c_double), ("pitch", C.c_double),
                 ("xi", C.c_double), ("gamma1", C.c_double), ("g", C.c_double * 3),
                 ("anchoring", C.c_int), ("W0", C.c_double), ("fd_ratio", C.c_int),
-                ("precision", C.c_int), ("coupling", C.c_int)]
+                ("precision", C.c_int), ("coupling", C.c_int), ("alpha", C.c_double * 6)]
 
 
 class OracleError(RuntimeError):
@@ -42,6 +42,8 @@ def _load():
         lib.nh_oracle_director_rhs.argtypes = [C.c_int] * 4 + [C.c_double] * 4 + [dp, dp, dp]
         lib.nh_oracle_elastic_stress.argtypes = [C.c_int] * 4 + [C.c_double] * 2 + [dp, dp]
         lib.nh_oracle_elastic_force.argtypes = [C.c_int] * 4 + [C.c_double] * 2 + [dp, dp]
+        lib.nh_oracle_viscous_stress.argtypes = [C.c_int] * 4 + [C.c_double] * 4 + [dp, dp, dp, dp]
+        lib.nh_oracle_lc_force.argtypes = [C.c_int] * 4 + [C.c_double] * 4 + [dp, dp, dp, dp]
         _lib = lib
     return _lib
 
@@ -70,10 +72,10 @@ class Oracle:
     """One oracle lattice; same call surface as the CUDA binding (init / set_director / step / get_fields)."""
 
     def __init__(self, nx, ny, nz, tau, K=0.0, pitch=0.0, xi=0.0, gamma1=1.0, g=(0.0, 0.0, 0.0),
-                 anchoring=0, W0=0.0, fd_ratio=1, precision=0, coupling=3, **_ignored):
+                 anchoring=0, W0=0.0, fd_ratio=1, precision=0, coupling=3, alpha=(0.0,) * 6, **_ignored):
         lib = _load()
         self.p = _Params(nx, ny, nz, tau, K, pitch, xi, gamma1, (C.c_double * 3)(*g), anchoring, W0,
-                         fd_ratio, precision, coupling)
+                         fd_ratio, precision, coupling, (C.c_double * 6)(*alpha))
         self.shape = (nz, ny, nx)
         self._h = C.c_void_p()
         _check(lib.nh_oracle_init_lattice(C.byref(self.p), C.byref(self._h)))
@@ -149,4 +151,28 @@ def elastic_force(n, K, q0, periodic_z=False):
     F = np.empty_like(n)
     nx, ny, nz = _dims(n)
     _check(_load().nh_oracle_elastic_force(nx, ny, nz, int(periodic_z), K, q0, _ptr(n), _ptr(F)))
+    return F
+
+
+def viscous_stress(n, u, K, q0, xi, gamma1, alpha, periodic_z=False):
+    """Leslie viscous stress (Eq. 3 with alpha4', N from Eq. 9); alpha = (a1, a2, a3, a4', a5, a6)."""
+    n = np.ascontiguousarray(n, dtype=np.float64)
+    u = _f64(u, n.shape)
+    al = np.ascontiguousarray(alpha, dtype=np.float64)
+    nx, ny, nz = _dims(n)
+    s = np.empty((9, nz, ny, nx))
+    _check(_load().nh_oracle_viscous_stress(nx, ny, nz, int(periodic_z), K, q0, xi, gamma1, _ptr(al),
+                                            _ptr(n), _ptr(u), _ptr(s)))
+    return s.reshape(3, 3, nz, ny, nx)
+
+
+def lc_force(n, u, K, q0, xi, gamma1, alpha, periodic_z=False):
+    """F^LC = d_b (sigma^e + sigma^v)_ab, Eq. 12."""
+    n = np.ascontiguousarray(n, dtype=np.float64)
+    u = _f64(u, n.shape)
+    al = np.ascontiguousarray(alpha, dtype=np.float64)
+    F = np.empty_like(n)
+    nx, ny, nz = _dims(n)
+    _check(_load().nh_oracle_lc_force(nx, ny, nz, int(periodic_z), K, q0, xi, gamma1, _ptr(al),
+                                      _ptr(n), _ptr(u), _ptr(F)))
     return F
