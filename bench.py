@@ -43,6 +43,8 @@ def parse():
     ap.add_argument("--two-step", action="store_true", help="NH_OPT_LB_TWOSTEP: force two LB steps per launch through the L2")
     ap.add_argument("--one-step", action="store_true", help="NH_OPT_LB_ONESTEP: one LB step per launch")
     ap.add_argument("--block-order", action="store_true", help="NH_OPT_LB_BLOCKORDER: two-step units in blockIdx order")
+    ap.add_argument("--leslie", type=float, default=0.0,
+                    help="scale of the paper's Table-1 Leslie viscosities in the force (row f1; 0 = elastic stress only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -54,6 +56,10 @@ def workload(args):
     if args.config == 4 and args.size:
         over["size"] = tuple(args.size)
     p = I.config(args.config, **over)
+    if args.leslie:
+        # alpha1..alpha6 of MBBA in simulation units as printed in the paper's Table 1
+        table1 = (0.0373, -0.4496, -0.0203, 0.9318, 0.3084, -0.1617)
+        p["alpha"] = tuple(args.leslie * a for a in table1)
     d = p.pop("director")
     p.pop("steps")
     name = {0: "configs[0] tiny channel", 1: "configs[1] single skyrmion tube", 2: "configs[2] precision sweep domain",
@@ -61,6 +67,8 @@ def workload(args):
     desc = {"workload": "%s %dx%dx%d" % (name, p["nx"], p["ny"], p["nz"]), "grid": [p["nx"], p["ny"], p["nz"]],
             "fd_ratio": p["fd_ratio"], "tau": p["tau"], "K": p["K"], "pitch": p["pitch"], "xi": p["xi"],
             "g_x": p["g"][0], "precision": args.precision}
+    if args.leslie:
+        desc["leslie_viscous_stress"] = "Table 1 x %g" % args.leslie
     return p, d, desc
 
 

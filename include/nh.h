@@ -12,6 +12,7 @@
  *                                                          PAPER.md:70-73, 81 (Eqs. 7-8, 10)
  *   force    : F^LC_a = d_b sigma_ab,  sigma = elastic (Ericksen) stress
  *                                                          PAPER.md:66 (Eq. 6), 97 (Eq. 12, last term)
+ *              optionally + the Leslie viscous stress      PAPER.md:50 (Eq. 3), 97-99 (Eq. 12)
  *   schedule : LB every step; director + force after every r-th step with Delta t_FD = r
  *                                                          PAPER.md:191-207 (Sec. II.D, Fig. 1)
  *
@@ -63,6 +64,12 @@ typedef struct {
   int    fd_ratio;     /* default r = Delta t_FD / Delta t_LB, >= 0 */
   int    precision;    /* NH_FP64_SHIFTED .. NH_FP64_UNSHIFTED */
   int    coupling;     /* bit0: F^LC acts on the flow; bit1: the flow acts on n   (3 = paper)  */
+  double alpha[6];     /* Leslie viscosities alpha1, alpha2, alpha3, alpha4', alpha5, alpha6 of the viscous
+                          stress inside F^LC (Eq. 3 with alpha4 -> alpha4', Eq. 12); N of Eq. 4 is taken
+                          from Eq. 9 as (h/gamma1 + xi n.D) perpendicular to n (reading G22).
+                          All 0 (the north_star's reduced model): elastic stress only.  xi and gamma1 are
+                          NOT derived from them (gamma1 = alpha3 - alpha2, gamma2 = alpha3 + alpha2 is
+                          the caller's business) */
 } nh_params;
 
 /* Bytes of device memory the lattice needs for these parameters (0 if they are invalid).

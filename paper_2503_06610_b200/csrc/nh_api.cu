@@ -50,6 +50,7 @@ const char* check_params(const nh_params* p) {
   if (p->precision < 0 || p->precision > 3) return "precision must be 0..3";
   if (p->anchoring != 0 || p->W0 != 0.0) return "only anchoring = 0 and W0 = 0 are built";
   if (p->coupling < 0 || p->coupling > 3) return "coupling must be 0..3";
+  for (int i = 0; i < 6; ++i) if (!std::isfinite(p->alpha[i])) return "alpha must be finite";
   return nullptr;
 }
 
@@ -179,6 +180,8 @@ nh::FdConst<T> fd_const(const nh_lattice* L, int r) {
   C.inv_gamma1 = (T)(1.0 / L->p.gamma1);
   C.xi = (T)L->p.xi;
   C.dt = (T)r;
+  C.visc = 0;
+  for (int i = 0; i < 6; ++i) { C.al[i] = (T)L->p.alpha[i]; if (L->p.alpha[i] != 0.0) C.visc = 1; }
   return C;
 }
 
@@ -358,21 +361,33 @@ bool tiles_fit(const nh_lattice* L) {
   return g.grid.y <= 65535u && g.grid.z <= 65535u;
 }
 
+bool viscous(const nh_lattice* L) {
+  for (int i = 0; i < 6; ++i) if (L->p.alpha[i] != 0.0) return true;
+  return false;
+}
+
+// F^LC from the current director and, with the viscous stress, the velocity in L->u (Eq. 12)
 template <typename T>
 int launch_force(nh_lattice* L) {
   Bracket br(L, KC_FORCE);
   if (br.rc) return br.rc;
+  const nh::FdConst<T> C = fd_const<T>(L, 1);
+  const T* n = (const T*)L->n[L->ncur];
+  const T* u = (const T*)L->u;
   if (!(L->options & NH_OPT_FD_DIRECT) && tiles_fit(L)) {
     const TileGrid g = tile_grid(L);
-    if (tiles_vec(L))
-      nh::force_tile_kernel<T, true><<<g.grid, nh::TILE_THREADS, nh::force_smem_bytes<T>(), L->stream>>>(
-          (const T*)L->n[L->ncur], (T*)L->F, L->G, fd_const<T>(L, 1), g.zchunk);
-    else
-      nh::force_tile_kernel<T, false><<<g.grid, nh::TILE_THREADS, nh::force_smem_bytes<T>(), L->stream>>>(
-          (const T*)L->n[L->ncur], (T*)L->F, L->G, fd_const<T>(L, 1), g.zchunk);
+    const bool vec = tiles_vec(L);
+    if (C.visc) {
+      const size_t sm = nh::force_smem_bytes<T, true>();
+      if (vec) nh::force_tile_kernel<T, true, true><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(n, u, (T*)L->F, L->G, C, g.zchunk);
+      else nh::force_tile_kernel<T, false, true><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(n, u, (T*)L->F, L->G, C, g.zchunk);
+    } else {
+      const size_t sm = nh::force_smem_bytes<T, false>();
+      if (vec) nh::force_tile_kernel<T, true, false><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(n, u, (T*)L->F, L->G, C, g.zchunk);
+      else nh::force_tile_kernel<T, false, false><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(n, u, (T*)L->F, L->G, C, g.zchunk);
+    }
   } else {
-    nh::force_direct_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
-        (const T*)L->n[L->ncur], (T*)L->F, L->G, fd_const<T>(L, 1));
+    nh::force_direct_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(n, u, (T*)L->F, L->G, C);
   }
   br.end();
   return NH_OK;
@@ -418,14 +433,17 @@ int launch_director(nh_lattice* L, int r) {
 // opt in to the dynamic shared memory the tiled kernels ask for (once per process and type)
 template <typename T>
 int enable_tile_smem() {
-  const int db = (int)nh::director_smem_bytes<T>(), fb = (int)nh::force_smem_bytes<T>();
+  const int db = (int)nh::director_smem_bytes<T>(), fb = (int)nh::force_smem_bytes<T, false>();
+  const int fvb = (int)nh::force_smem_bytes<T, true>();
   const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
   NH_CUDA(cudaFuncSetAttribute(nh::director_tile_kernel<T, 0, true>, attr, db));
   NH_CUDA(cudaFuncSetAttribute(nh::director_tile_kernel<T, 1, true>, attr, db));
   NH_CUDA(cudaFuncSetAttribute(nh::director_tile_kernel<T, 0, false>, attr, db));
   NH_CUDA(cudaFuncSetAttribute(nh::director_tile_kernel<T, 1, false>, attr, db));
-  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, true>, attr, fb));
-  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false>, attr, fb));
+  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, true, false>, attr, fb));
+  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false, false>, attr, fb));
+  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, true, true>, attr, fvb));
+  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false, true>, attr, fvb));
   return NH_OK;
 }
 
@@ -446,7 +464,8 @@ int step_typed(nh_lattice* L, int n_lb, int r) {
     L->cur ^= 1;
     L->t += 1;
     if (r > 0 && L->t % r == 0) {
-      if (L->p.coupling & 2) { rc = launch_velocity<T, SH>(L); if (rc) return rc; }
+      // u(t): for the director equation (coupling bit1) and for the viscous stress in the force
+      if ((L->p.coupling & 2) || viscous(L)) { rc = launch_velocity<T, SH>(L); if (rc) return rc; }
       rc = launch_director<T>(L, r); if (rc) return rc;
       rc = launch_force<T>(L); if (rc) return rc;
     }
@@ -487,7 +506,7 @@ int init_typed(nh_lattice* L) {
   return NH_OK;
 }
 
-template <typename T>
+template <typename T, bool SH>
 int set_director_typed(nh_lattice* L) {
   const size_t N = L->G.N;
   {
@@ -495,7 +514,9 @@ int set_director_typed(nh_lattice* L) {
     nh::store_director_kernel<T><<<blocks_for(N), BLOCK, 0, L->stream>>>(
         L->stage, (T*)L->n[L->ncur], (T*)L->nP, (T*)L->n[L->ncur ^ 1], L->G);
   }
-  return launch_force<T>(L);  // reading G9: force from the initial director
+  // reading G9: force from the initial director (the viscous part from the current velocity)
+  if (viscous(L)) { const int rc = launch_velocity<T, SH>(L); if (rc) return rc; }
+  return launch_force<T>(L);
 }
 
 template <typename T, bool SH>
@@ -682,8 +703,12 @@ int nh_set_director(nh_lattice* L, const double* n_host) {
   NH_CUDA(cudaStreamSynchronize(L->stream));
   if (flag) return fail(NH_EINVAL, "zero-length or non-finite director vector");
   int rc;
-  if (word_of(L->p.precision) == 8) rc = set_director_typed<double>(L);
-  else rc = set_director_typed<float>(L);
+  switch (L->p.precision) {
+    case NH_FP64_SHIFTED: rc = set_director_typed<double, true>(L); break;
+    case NH_FP32_SHIFTED: rc = set_director_typed<float, true>(L); break;
+    case NH_FP32_UNSHIFTED: rc = set_director_typed<float, false>(L); break;
+    default: rc = set_director_typed<double, false>(L); break;
+  }
   if (rc) return rc;
   NH_CUDA(cudaGetLastError());
   NH_CUDA(cudaStreamSynchronize(L->stream));

@@ -20,6 +20,8 @@ struct FdConst {
   T inv_gamma1; // 1/gamma1
   T xi;         // flow alignment
   T dt;         // Delta t_FD = r
+  T al[6];      // Leslie viscosities alpha1, alpha2, alpha3, alpha4', alpha5, alpha6 (Eqs. 3, 12)
+  int visc;     // any of them non-zero: the force includes the viscous stress
 };
 
 template <typename T> struct V3 { T x, y, z; };
@@ -143,30 +145,66 @@ __device__ __forceinline__ V3<T> stress_column(const FdConst<T>& C, int b, V3<T>
   return {C.Kq0 * qx - C.K * dot(dxn, db), C.Kq0 * qy - C.K * dot(dyn, db), C.Kq0 * qz - C.K * dot(dzn, db)};
 }
 
+// Leslie viscous stress, Eq. 3 with alpha4 -> alpha4' as in the force of Eq. 12
+// (PAPER.md:97-99), added column by column: s?[a] += sigma^v_{a ?},
+//   sigma^v_ab = a1 n_a n_b (n.D.n) + a2 n_b N_a + a3 n_a N_b + a4' D_ab + a5 n_b (n.D)_a + a6 n_a (n.D)_b
+// D as printed in Eq. 5; N of Eq. 4 from Eq. 9: N = h/gamma1 + xi n.D, projected perpendicular
+// to n (reading G22); h = K lap n - 2 K q0 curl n as in the director equation.
+// d?n, d?u: central differences; lap: 7-point Laplacian of n.
+template <typename T>
+__device__ __forceinline__ void viscous_add(const FdConst<T>& C, V3<T> n, V3<T> dxn, V3<T> dyn, V3<T> dzn,
+                                            V3<T> lap, V3<T> dxu, V3<T> dyu, V3<T> dzu,
+                                            V3<T>& sx, V3<T>& sy, V3<T>& sz) {
+  const T h2 = T(0.5);
+  const T Dxy = h2 * (dxu.y + dyu.x), Dxz = h2 * (dxu.z + dzu.x), Dyz = h2 * (dyu.z + dzu.y);
+  const V3<T> Dx = {dxu.x, Dxy, Dxz}, Dy = {Dxy, dyu.y, Dyz}, Dz = {Dxz, Dyz, dzu.z};   // columns = rows
+  const V3<T> nD = {dot(n, Dx), dot(n, Dy), dot(n, Dz)};
+  const V3<T> curl = {dyn.z - dzn.y, dzn.x - dxn.z, dxn.y - dyn.x};
+  const V3<T> A = C.inv_gamma1 * (C.K * lap - (T(2) * C.Kq0) * curl) + C.xi * nD;
+  const V3<T> N = A - dot(n, A) * n;
+  const T nnD = dot(n, nD);
+  const V3<T> w = C.al[1] * N + C.al[4] * nD;                  // multiplies n_b
+  sx = sx + (C.al[0] * n.x * nnD + C.al[2] * N.x + C.al[5] * nD.x) * n + n.x * w + C.al[3] * Dx;
+  sy = sy + (C.al[0] * n.y * nnD + C.al[2] * N.y + C.al[5] * nD.y) * n + n.y * w + C.al[3] * Dy;
+  sz = sz + (C.al[0] * n.z * nnD + C.al[2] * N.z + C.al[5] * nD.z) * n + n.z * w + C.al[3] * Dz;
+}
+
 // sigma_{. b} at the cell (x, y, z) read from global memory; zero on the plate layers (reading G6).
 template <typename T>
 __device__ __forceinline__ V3<T> stress_column_at(const FdConst<T>& C, int b, const T* __restrict__ n,
-                                                  const Geom& G, int x, int y, int z) {
+                                                  const T* __restrict__ u, const Geom& G, int x, int y, int z) {
   if (z == 0 || z == G.nz - 1) return {T(0), T(0), T(0)};
   const Nbr q = neighbours(G, x, y, z);
   const T h = T(0.5);
-  return stress_column(C, b, ld3(n, G.N, q.c), h * (ld3(n, G.N, q.xp) - ld3(n, G.N, q.xm)),
-                       h * (ld3(n, G.N, q.yp) - ld3(n, G.N, q.ym)), h * (ld3(n, G.N, q.zp) - ld3(n, G.N, q.zm)));
+  const V3<T> nc = ld3(n, G.N, q.c);
+  const V3<T> nxp = ld3(n, G.N, q.xp), nxm = ld3(n, G.N, q.xm), nyp = ld3(n, G.N, q.yp), nym = ld3(n, G.N, q.ym);
+  const V3<T> nzp = ld3(n, G.N, q.zp), nzm = ld3(n, G.N, q.zm);
+  const V3<T> dxn = h * (nxp - nxm), dyn = h * (nyp - nym), dzn = h * (nzp - nzm);
+  V3<T> s = stress_column(C, b, nc, dxn, dyn, dzn);
+  if (C.visc) {
+    const V3<T> lap = ((nxp + nxm) + (nyp + nym)) + (nzp + nzm) - T(6) * nc;
+    const V3<T> dxu = h * (ld3(u, G.N, q.xp) - ld3(u, G.N, q.xm)), dyu = h * (ld3(u, G.N, q.yp) - ld3(u, G.N, q.ym));
+    const V3<T> dzu = h * (ld3(u, G.N, q.zp) - ld3(u, G.N, q.zm));
+    V3<T> vx = {T(0), T(0), T(0)}, vy = vx, vz = vx;
+    viscous_add(C, nc, dxn, dyn, dzn, lap, dxu, dyu, dzu, vx, vy, vz);
+    s = s + (b == 0 ? vx : (b == 1 ? vy : vz));
+  }
+  return s;
 }
 
-// Force (Eq. 12, last term): F_a = sum_b [sigma_ab(x + e_b) - sigma_ab(x - e_b)]/2.
+// Force (Eq. 12): F_a = sum_b [sigma_ab(x + e_b) - sigma_ab(x - e_b)]/2, sigma = sigma^e (+ sigma^v).
 template <typename T>
 __global__ void __launch_bounds__(256)
-force_direct_kernel(const T* __restrict__ n, T* __restrict__ F, Geom G, FdConst<T> C) {
+force_direct_kernel(const T* __restrict__ n, const T* __restrict__ u, T* __restrict__ F, Geom G, FdConst<T> C) {
   const unsigned k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= G.nfluid) return;
   int x, y, z;
   cell_of(k, G, x, y, z);
   const int xm = (x == 0) ? G.nx - 1 : x - 1, xp = (x == G.nx - 1) ? 0 : x + 1;
   const int ym = (y == 0) ? G.ny - 1 : y - 1, yp = (y == G.ny - 1) ? 0 : y + 1;
-  V3<T> f = stress_column_at(C, 0, n, G, xp, y, z) - stress_column_at(C, 0, n, G, xm, y, z);
-  f = f + (stress_column_at(C, 1, n, G, x, yp, z) - stress_column_at(C, 1, n, G, x, ym, z));
-  f = f + (stress_column_at(C, 2, n, G, x, y, z + 1) - stress_column_at(C, 2, n, G, x, y, z - 1));
+  V3<T> f = stress_column_at(C, 0, n, u, G, xp, y, z) - stress_column_at(C, 0, n, u, G, xm, y, z);
+  f = f + (stress_column_at(C, 1, n, u, G, x, yp, z) - stress_column_at(C, 1, n, u, G, x, ym, z));
+  f = f + (stress_column_at(C, 2, n, u, G, x, y, z + 1) - stress_column_at(C, 2, n, u, G, x, y, z - 1));
   const size_t c = (size_t)k + G.plane;
   F[c] = T(0.5) * f.x; F[G.N + c] = T(0.5) * f.y; F[2 * G.N + c] = T(0.5) * f.z;
 }

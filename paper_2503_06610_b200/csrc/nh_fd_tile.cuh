@@ -236,9 +236,9 @@ constexpr int FORCE_SLOTS = 4;
 struct SigShape {                       // sigma_.x / sigma_.y plane: [2 columns][3][TY+2][TX+2]
   static constexpr int PX = TX + 2, PY = TY + 2, CELLS = PX * PY, ELEMS = 6 * CELLS;
 };
-template <typename T>
+template <typename T, bool VISC = false>
 constexpr size_t force_smem_bytes() {
-  return ((size_t)FORCE_SLOTS * PlaneShape<2>::ELEMS + 2 * SigShape::ELEMS) * sizeof(T);
+  return ((size_t)(VISC ? 2 : 1) * FORCE_SLOTS * PlaneShape<2>::ELEMS + 2 * SigShape::ELEMS) * sizeof(T);
 }
 
 // grad n at the staged position `o` of plane slots (zm, c, zp)
@@ -251,6 +251,30 @@ __device__ __forceinline__ void grad_staged(const T* pzm, const T* pc, const T* 
   dxn = h * (lds3<T, 2>(pc, o + 1) - lds3<T, 2>(pc, o - 1));
   dyn = h * (lds3<T, 2>(pc, o + S::RS) - lds3<T, 2>(pc, o - S::RS));
   dzn = h * (lds3<T, 2>(pzp, o) - lds3<T, 2>(pzm, o));
+}
+// the same plus the 7-point Laplacian (the viscous stress needs the molecular field)
+template <typename T>
+__device__ __forceinline__ void grad_lap_staged(const T* pzm, const T* pc, const T* pzp, int o,
+                                                V3<T>& n, V3<T>& dxn, V3<T>& dyn, V3<T>& dzn, V3<T>& lap) {
+  using S = PlaneShape<2>;
+  const T h = T(0.5);
+  n = lds3<T, 2>(pc, o);
+  const V3<T> xp = lds3<T, 2>(pc, o + 1), xm = lds3<T, 2>(pc, o - 1);
+  const V3<T> yp = lds3<T, 2>(pc, o + S::RS), ym = lds3<T, 2>(pc, o - S::RS);
+  const V3<T> zp = lds3<T, 2>(pzp, o), zm = lds3<T, 2>(pzm, o);
+  dxn = h * (xp - xm); dyn = h * (yp - ym); dzn = h * (zp - zm);
+  lap = ((xp + xm) + (yp + ym)) + (zp + zm) - T(6) * n;
+}
+// sigma^e + sigma^v at the staged position `o`: all three columns
+template <typename T>
+__device__ __forceinline__ void stress_visc_staged(const FdConst<T>& C, const T* nzm, const T* nc, const T* nzp,
+                                                   const T* uzm, const T* uc, const T* uzp, int o,
+                                                   V3<T>& sx, V3<T>& sy, V3<T>& sz) {
+  V3<T> n, dxn, dyn, dzn, lap, u0, dxu, dyu, dzu;
+  grad_lap_staged(nzm, nc, nzp, o, n, dxn, dyn, dzn, lap);
+  grad_staged(uzm, uc, uzp, o, u0, dxu, dyu, dzu);
+  stress_all(C, n, dxn, dyn, dzn, sx, sy, sz);
+  viscous_add(C, n, dxn, dyn, dzn, lap, dxu, dyu, dzu, sx, sy, sz);
 }
 
 // All three columns of sigma at once: c_a = n x d_a n,  g_ab = d_a n . d_b n (symmetric),
@@ -266,13 +290,17 @@ __device__ __forceinline__ void stress_all(const FdConst<T>& C, V3<T> n, V3<T> d
   sz = {C.Kq0 * cx.z - C.K * gxz, C.Kq0 * cy.z - C.K * gyz, C.Kq0 * cz.z - C.K * gzz};
 }
 
-template <typename T, bool VEC>
+// VISC: the Leslie viscous stress is added (Eq. 12 in full, row f1): u is staged like n.
+template <typename T, bool VEC, bool VISC>
 __global__ void __launch_bounds__(TILE_THREADS)
-force_tile_kernel(const T* __restrict__ n, T* __restrict__ Fout, Geom G, FdConst<T> C, int zchunk) {
+force_tile_kernel(const T* __restrict__ n, const T* __restrict__ u, T* __restrict__ Fout, Geom G,
+                  FdConst<T> C, int zchunk) {
   using S = PlaneShape<2>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* sn = reinterpret_cast<T*>(smem_raw);                 // [FORCE_SLOTS][S::ELEMS]
   T* ssig = sn + FORCE_SLOTS * S::ELEMS;                  // [2][SigShape::ELEMS]
+  T* su = ssig + 2 * SigShape::ELEMS;                     // [FORCE_SLOTS][S::ELEMS] (VISC only)
+  const unsigned su_addr = smem_u32(su);
   const int tx = threadIdx.x % TX, ty = threadIdx.x / TX;
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
   const int z0 = 1 + blockIdx.z * zchunk;
@@ -302,7 +330,12 @@ force_tile_kernel(const T* __restrict__ n, T* __restrict__ Fout, Geom G, FdConst
   const int zlo = max(pfirst - 1, 0), zhi = min(plast + 1, G.nz - 1);
   int zf = zlo;                                            // next plane to fetch
   const T* src = n + (size_t)zlo * G.plane;
-  for (; zf <= zlo + 2; ++zf) { st.fetch(src, sn_addr + (zf & 3) * SLOT_BYTES); src += G.plane; }
+  const T* usrc = u + (size_t)zlo * G.plane;
+  for (; zf <= zlo + 2; ++zf) {
+    st.fetch(src, sn_addr + (zf & 3) * SLOT_BYTES);
+    if (VISC) { st.fetch(usrc, su_addr + (zf & 3) * SLOT_BYTES); usrc += G.plane; }
+    src += G.plane;
+  }
   cp_async_commit();
   const V3<T> zero = {T(0), T(0), T(0)};
   V3<T> szA = zero, szB = zero;                           // sigma_.z at planes p-2, p-1
@@ -314,6 +347,7 @@ force_tile_kernel(const T* __restrict__ n, T* __restrict__ Fout, Geom G, FdConst
     __syncthreads();
     if (zf <= zhi && zf <= p + 2) {                        // keep one plane ahead of p+1
       st.fetch(src, sn_addr + (zf & 3) * SLOT_BYTES);
+      if (VISC) { st.fetch(usrc, su_addr + (zf & 3) * SLOT_BYTES); usrc += G.plane; }
       src += G.plane; ++zf;
     }
     cp_async_commit();
@@ -331,13 +365,27 @@ force_tile_kernel(const T* __restrict__ n, T* __restrict__ Fout, Geom G, FdConst
       const T* pc = sn + (p & 3) * S::ELEMS;
       const T* pzp = sn + ((p + 1) & 3) * S::ELEMS;
       V3<T> nn, dxn, dyn, dzn, sx, sy;
-      grad_staged(pzm, pc, pzp, on, nn, dxn, dyn, dzn);
-      stress_all(C, nn, dxn, dyn, dzn, sx, sy, szC);
+      const T* uzm = su + ((p - 1) & 3) * S::ELEMS;
+      const T* uc = su + (p & 3) * S::ELEMS;
+      const T* uzp = su + ((p + 1) & 3) * S::ELEMS;
+      if (VISC) {
+        stress_visc_staged(C, pzm, pc, pzp, uzm, uc, uzp, on, sx, sy, szC);
+      } else {
+        grad_staged(pzm, pc, pzp, on, nn, dxn, dyn, dzn);
+        stress_all(C, nn, dxn, dyn, dzn, sx, sy, szC);
+      }
       sig[0 * SigShape::CELLS + os] = sx.x; sig[1 * SigShape::CELLS + os] = sx.y; sig[2 * SigShape::CELLS + os] = sx.z;
       sig[3 * SigShape::CELLS + os] = sy.x; sig[4 * SigShape::CELLS + os] = sy.y; sig[5 * SigShape::CELLS + os] = sy.z;
       if (hn >= 0) {
-        grad_staged(pzm, pc, pzp, hn, nn, dxn, dyn, dzn);
-        const V3<T> sh = stress_column(C, hcol, nn, dxn, dyn, dzn);
+        V3<T> sh;
+        if (VISC) {
+          V3<T> hx, hy, hz;
+          stress_visc_staged(C, pzm, pc, pzp, uzm, uc, uzp, hn, hx, hy, hz);
+          sh = hcol == 0 ? hx : hy;
+        } else {
+          grad_staged(pzm, pc, pzp, hn, nn, dxn, dyn, dzn);
+          sh = stress_column(C, hcol, nn, dxn, dyn, dzn);
+        }
         sig[0 * SigShape::CELLS + hs] = sh.x;
         sig[1 * SigShape::CELLS + hs] = sh.y;
         sig[2 * SigShape::CELLS + hs] = sh.z;
