@@ -52,6 +52,7 @@ int opposite(int i) { return TAB.opp[i]; }
 struct Grid {
   int nx, ny, nz;
   bool pz;  // periodic in z (pins only)
+  double W0 = 0.0;  // bulk anchoring strength (row f3, reading G14): energy -(W0/2) (n.z_hat)^2 per cell
   size_t N() const { return (size_t)nx * ny * nz; }
   size_t at(int x, int y, int z) const { return ((size_t)z * ny + y) * nx + x; }
   int wx(int x) const { return (x + nx) % nx; }  // periodic x, y
@@ -97,6 +98,8 @@ void molecular_field_cell(const Grid& G, double K, double q0, const double* m, i
       lap += m[c * N + G.nb(x, y, z, b, +1)] + m[c * N + G.nb(x, y, z, b, -1)] - 2.0 * m[c * N + c0];
     h[c] = K * lap - 2.0 * K * q0 * curl[c];
   }
+  // bulk effective anchoring along z (its form is reading G14): h_z += W0 n_z
+  h[2] += G.W0 * m[2 * N + c0];
 }
 
 // Right-hand side of the director equation, Eq. 9, with xi = -gamma2/gamma1 (G4),
@@ -388,6 +391,21 @@ struct nh_oracle_lattice {
           const double len = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
           for (int a = 0; a < 3; ++a) dst[a * N + c] = v[a] / len;  // renormalise (G3)
         }
+    mirror_plates(dst);
+  }
+
+  // Free plates (anchoring = 1, "no anchoring at the plates"; reading G23): the plate
+  // layers carry no director of their own, they copy the adjacent fluid layer (zero normal
+  // derivative), so the stencils at z = 1 and z = nz-2 see no anchoring torque.
+  void mirror_plates(std::vector<double>& m) const {
+    if (p.anchoring != 1) return;
+    const size_t N = G.N();
+    for (int a = 0; a < 3; ++a)
+      for (int y = 0; y < G.ny; ++y)
+        for (int x = 0; x < G.nx; ++x) {
+          m[a * N + G.at(x, y, 0)] = m[a * N + G.at(x, y, 1)];
+          m[a * N + G.at(x, y, G.nz - 1)] = m[a * N + G.at(x, y, G.nz - 2)];
+        }
   }
 
   // F^LC from the current director (and, for the viscous part, the current velocity).
@@ -435,12 +453,14 @@ int nh_oracle_init_lattice(const nh_oracle_params* p, nh_oracle_lattice** out) {
   if (p->K < 0.0) return fail(E_INVAL, "K must be >= 0");
   if (p->fd_ratio < 0) return fail(E_INVAL, "fd_ratio must be >= 0");
   if (p->precision < 0 || p->precision > 3) return fail(E_INVAL, "precision must be 0..3");
-  if (p->anchoring != 0 || p->W0 != 0.0) return fail(E_INVAL, "only anchoring = 0, W0 = 0 are built");
+  if (p->anchoring != 0 && p->anchoring != 1) return fail(E_INVAL, "anchoring must be 0 (homeotropic plates) or 1 (free plates)");
+  if (!std::isfinite(p->W0)) return fail(E_INVAL, "W0 must be finite");
   nh_oracle_lattice* L = new (std::nothrow) nh_oracle_lattice();
   if (!L) return fail(E_NOMEM, "out of memory");
   try {
     L->p = *p;
     L->G = Grid{p->nx, p->ny, p->nz, false};
+    L->G.W0 = p->W0;
     L->q0 = p->pitch > 0.0 ? 2.0 * M_PI / p->pitch : 0.0;
     L->shifted = (p->precision == 0 || p->precision == 1);
     L->t = 0;
@@ -484,8 +504,10 @@ int nh_oracle_set_director(nh_oracle_lattice* L, const double* n_host) {
     L->n[N + c] = b / len;
     L->n[2 * N + c] = d / len;
   }
-  // infinite homeotropic anchoring: plate layers hold z_hat and never change
-  for (int zz = 0; zz < 2; ++zz) {
+  // infinite homeotropic anchoring: plate layers hold z_hat and never change;
+  // free plates (anchoring = 1): they copy the adjacent fluid layer instead
+  L->mirror_plates(L->n);
+  for (int zz = 0; zz < 2 && L->p.anchoring == 0; ++zz) {
     const int z = zz == 0 ? 0 : L->G.nz - 1;
     for (int y = 0; y < L->G.ny; ++y)
       for (int x = 0; x < L->G.nx; ++x) {
@@ -554,6 +576,23 @@ int nh_oracle_molecular_field(int nx, int ny, int nz, int periodic_z, double K, 
                               const double* n, double* h) {
   if (!n || !h || bad_dims(nx, ny, nz)) return fail(E_INVAL, "bad arguments");
   const Grid G{nx, ny, nz, periodic_z != 0};
+  const size_t N = G.N();
+  std::memset(h, 0, sizeof(double) * 3 * N);
+  for (int z = G.z_lo(); z < G.z_hi(); ++z)
+    for (int y = 0; y < ny; ++y)
+      for (int x = 0; x < nx; ++x) {
+        double hh[3];
+        molecular_field_cell(G, K, q0, n, x, y, z, hh);
+        for (int c = 0; c < 3; ++c) h[c * N + G.at(x, y, z)] = hh[c];
+      }
+  return 0;
+}
+
+int nh_oracle_molecular_field_w0(int nx, int ny, int nz, int periodic_z, double K, double q0, double W0,
+                                 const double* n, double* h) {
+  if (!n || !h || bad_dims(nx, ny, nz)) return fail(E_INVAL, "bad arguments");
+  Grid G{nx, ny, nz, periodic_z != 0};
+  G.W0 = W0;
   const size_t N = G.N();
   std::memset(h, 0, sizeof(double) * 3 * N);
   for (int z = G.z_lo(); z < G.z_hi(); ++z)

@@ -48,8 +48,10 @@ typedef struct {
   double xi;           /* flow alignment = -gamma2/gamma1 (G4)   */
   double gamma1;       /* rotational viscosity > 0   */
   double g[3];         /* body acceleration */
-  int    anchoring;    /* 0 = homeotropic, fixed at both plates  */
-  double W0;           /* bulk anchoring (not built; must be 0)  */
+  int    anchoring;    /* 0 = homeotropic, fixed at both plates
+                          1 = free plates (no anchoring), reading G23  */
+  double W0;           /* bulk effective anchoring along z: h_z += W0 n_z (reading G14)
+                                                                            PAPER.md:229  */
   int    fd_ratio;     /* default Delta t_FD / Delta t_LB >= 0  */
   int    precision;    /* 0,1: shifted populations (Eqs. 19-23); 2,3: unshifted (Eqs. 14-17).
                           The oracle computes in FP64 whatever this says.                  */
@@ -77,6 +79,8 @@ int  nh_oracle_num_threads(void);
  *                 stencils read whatever the plate layers of the inputs hold.          */
 int nh_oracle_molecular_field(int nx, int ny, int nz, int periodic_z, double K, double q0,
                               const double* n, double* h);
+int nh_oracle_molecular_field_w0(int nx, int ny, int nz, int periodic_z, double K, double q0, double W0,
+                                 const double* n, double* h);   /* + the bulk anchoring term */
 int nh_oracle_director_rhs(int nx, int ny, int nz, int periodic_z, double K, double q0,
                            double xi, double gamma1, const double* n, const double* u, double* R);
 int nh_oracle_elastic_stress(int nx, int ny, int nz, int periodic_z, double K, double q0,

@@ -39,6 +39,7 @@ def _load():
         lib.nh_oracle_free.restype = None
         lib.nh_oracle_last_error.restype = C.c_char_p
         lib.nh_oracle_molecular_field.argtypes = [C.c_int] * 4 + [C.c_double] * 2 + [dp, dp]
+        lib.nh_oracle_molecular_field_w0.argtypes = [C.c_int] * 4 + [C.c_double] * 3 + [dp, dp]
         lib.nh_oracle_director_rhs.argtypes = [C.c_int] * 4 + [C.c_double] * 4 + [dp, dp, dp]
         lib.nh_oracle_elastic_stress.argtypes = [C.c_int] * 4 + [C.c_double] * 2 + [dp, dp]
         lib.nh_oracle_elastic_force.argtypes = [C.c_int] * 4 + [C.c_double] * 2 + [dp, dp]
@@ -120,11 +121,14 @@ def _dims(n):
     return nx, ny, nz
 
 
-def molecular_field(n, K, q0, periodic_z=False):
+def molecular_field(n, K, q0, periodic_z=False, W0=0.0):
     n = np.ascontiguousarray(n, dtype=np.float64)
     h = np.empty_like(n)
     nx, ny, nz = _dims(n)
-    _check(_load().nh_oracle_molecular_field(nx, ny, nz, int(periodic_z), K, q0, _ptr(n), _ptr(h)))
+    if W0:
+        _check(_load().nh_oracle_molecular_field_w0(nx, ny, nz, int(periodic_z), K, q0, W0, _ptr(n), _ptr(h)))
+    else:
+        _check(_load().nh_oracle_molecular_field(nx, ny, nz, int(periodic_z), K, q0, _ptr(n), _ptr(h)))
     return h
 
 

@@ -442,7 +442,8 @@ def test_plates_stay_fixed_and_set_director_normalises():
 
 def test_invalid_arguments_are_rejected():
     from oracle import OracleError
-    for bad in (dict(tau=0.5), dict(nz=2), dict(gamma1=0.0), dict(K=-1.0), dict(fd_ratio=-1), dict(W0=0.1)):
+    for bad in (dict(tau=0.5), dict(nz=2), dict(gamma1=0.0), dict(K=-1.0), dict(fd_ratio=-1), dict(W0=float("nan")),
+                dict(anchoring=2)):
         kw = dict(nx=4, ny=4, nz=5, tau=0.8)
         kw.update(bad)
         with pytest.raises(OracleError):
