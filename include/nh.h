@@ -24,7 +24,8 @@
  *     No exception or abort crosses this boundary.
  *   - Fields are arrays [component][z][y][x], x fastest, N = nx*ny*nz cells.  Layers z = 0 and
  *     z = nz-1 are the solid plates (wall half-way between layers 0|1 and nz-2|nz-1); the fluid is
- *     z = 1..nz-2.  On the plates rho = 1, u = 0, F^LC = 0 and n = z_hat are returned.
+ *     z = 1..nz-2.  On the plates rho = 1, u = 0, F^LC = 0 and n = z_hat (anchoring 0) or the copy
+ *     of the adjacent fluid layer (anchoring 1) are returned.
  *   - Every HOST array is FP64 whatever the device precision; conversion happens on the device.
  *   - Ownership: the caller owns all host arrays and the device workspace and keeps the workspace
  *     alive until nh_free.  The library owns only the handle.
@@ -59,8 +60,11 @@ typedef struct {
   double xi;           /* flow-alignment parameter = -gamma2/gamma1  */
   double gamma1;       /* rotational viscosity, > 0  */
   double g[3];         /* body acceleration; the force on the fluid is rho g  */
-  int    anchoring;    /* 0 = infinite homeotropic at both plates (only value built) PAPER.md:103 */
-  double W0;           /* bulk anchoring strength; must be 0 (not built) */
+  int    anchoring;    /* 0 = infinite homeotropic at both plates: n = z_hat there
+                          1 = free plates: the plate layers copy the adjacent fluid layer (zero
+                              normal derivative, no anchoring torque; G23) PAPER.md:229 */
+  double W0;           /* bulk effective anchoring along z: h_z += W0 n_z, from the energy
+                          -(W0/2) (n.z_hat)^2 per cell (G14) */
   int    fd_ratio;     /* default r = Delta t_FD / Delta t_LB, >= 0 */
   int    precision;    /* NH_FP64_SHIFTED .. NH_FP64_UNSHIFTED */
   int    coupling;     /* bit0: F^LC acts on the flow; bit1: the flow acts on n   (3 = paper)  */
@@ -85,7 +89,7 @@ int nh_init_lattice(const nh_params* p, void* dev_workspace, size_t bytes, void*
                     nh_lattice** out);
 
 /* Set the director from a HOST array [3][nz][ny][nx] (FP64).  Each vector is normalised, the plate
- * layers are overwritten with z_hat, n^P := n and F^LC is computed from it
+ * layers are overwritten with z_hat (anchoring 0) or with the adjacent fluid layer (anchoring 1), n^P := n and F^LC is computed from it
  * (Eq. 12; reading G9).  Populations and t are untouched.  NH_EINVAL if a vector has
  * zero or non-finite length (checked on the device; the lattice is then unchanged). */
 int nh_set_director(nh_lattice* L, const double* n_host);

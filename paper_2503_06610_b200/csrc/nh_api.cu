@@ -48,7 +48,8 @@ const char* check_params(const nh_params* p) {
   if (!std::isfinite(p->g[0]) || !std::isfinite(p->g[1]) || !std::isfinite(p->g[2])) return "g must be finite";
   if (p->fd_ratio < 0) return "fd_ratio must be >= 0";
   if (p->precision < 0 || p->precision > 3) return "precision must be 0..3";
-  if (p->anchoring != 0 || p->W0 != 0.0) return "only anchoring = 0 and W0 = 0 are built";
+  if (p->anchoring != 0 && p->anchoring != 1) return "anchoring must be 0 (homeotropic plates) or 1 (free plates)";
+  if (!std::isfinite(p->W0)) return "W0 must be finite";
   if (p->coupling < 0 || p->coupling > 3) return "coupling must be 0..3";
   for (int i = 0; i < 6; ++i) if (!std::isfinite(p->alpha[i])) return "alpha must be finite";
   return nullptr;
@@ -181,6 +182,7 @@ nh::FdConst<T> fd_const(const nh_lattice* L, int r) {
   C.xi = (T)L->p.xi;
   C.dt = (T)r;
   C.visc = 0;
+  C.W0 = (T)L->p.W0;
   for (int i = 0; i < 6; ++i) { C.al[i] = (T)L->p.alpha[i]; if (L->p.alpha[i] != 0.0) C.visc = 1; }
   return C;
 }
@@ -392,6 +394,17 @@ int launch_force(nh_lattice* L) {
   br.end();
   return NH_OK;
 }
+// free plates: the plate layers of a director array follow the adjacent fluid layers
+template <typename T>
+int mirror_plates(nh_lattice* L, void* field) {
+  if (L->p.anchoring != 1) return NH_OK;
+  Bracket br(L, KC_OTHER);
+  if (br.rc) return br.rc;
+  nh::mirror_plates_kernel<T><<<blocks_for(3 * (size_t)L->G.plane), BLOCK, 0, L->stream>>>((T*)field, L->G);
+  br.end();
+  return NH_OK;
+}
+
 template <typename T>
 int launch_director(nh_lattice* L, int r) {
   const int with_flow = (L->p.coupling & 2) ? 1 : 0;
@@ -412,6 +425,7 @@ int launch_director(nh_lattice* L, int r) {
           (const T*)L->n[L->ncur], (const T*)L->u, (T*)L->nP, L->G, C, with_flow);
     br.end();
   }
+  { const int rc = mirror_plates<T>(L, L->nP); if (rc) return rc; }
   {
     Bracket br(L, KC_CORR);
     if (br.rc) return br.rc;
@@ -427,7 +441,7 @@ int launch_director(nh_lattice* L, int r) {
     br.end();
   }
   L->ncur ^= 1;
-  return NH_OK;
+  return mirror_plates<T>(L, L->n[L->ncur]);
 }
 
 // opt in to the dynamic shared memory the tiled kernels ask for (once per process and type)
@@ -514,6 +528,7 @@ int set_director_typed(nh_lattice* L) {
     nh::store_director_kernel<T><<<blocks_for(N), BLOCK, 0, L->stream>>>(
         L->stage, (T*)L->n[L->ncur], (T*)L->nP, (T*)L->n[L->ncur ^ 1], L->G);
   }
+  for (void* fld : {L->n[0], L->n[1], L->nP}) { const int rc = mirror_plates<T>(L, fld); if (rc) return rc; }
   // reading G9: force from the initial director (the viscous part from the current velocity)
   if (viscous(L)) { const int rc = launch_velocity<T, SH>(L); if (rc) return rc; }
   return launch_force<T>(L);

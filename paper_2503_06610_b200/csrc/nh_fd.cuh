@@ -22,6 +22,7 @@ struct FdConst {
   T dt;         // Delta t_FD = r
   T al[6];      // Leslie viscosities alpha1, alpha2, alpha3, alpha4', alpha5, alpha6 (Eqs. 3, 12)
   int visc;     // any of them non-zero: the force includes the viscous stress
+  T W0;         // bulk anchoring along z: h_z += W0 n_z (reading G14)
 };
 
 template <typename T> struct V3 { T x, y, z; };
@@ -59,7 +60,7 @@ __device__ __forceinline__ Nbr neighbours(const Geom& G, int x, int y, int z) {
 }
 
 // Right-hand side of Eq. 9 at one cell from the centre value and the six neighbours of m and u.
-//   h   = K lap m - 2 K q0 curl m          (7-point Laplacian, central curl)
+//   h   = K lap m - 2 K q0 curl m + W0 m_z z_hat   (7-point Laplacian, central curl; bulk anchoring)
 //   R   = h/gamma1 + xi m.D - (u.grad) m + W.m,   D, W as printed in Eq. 5
 //   R  <- R - (m.R) m                      (reading G3)
 // d?m = central difference of m along ?, s?m = m(+) + m(-) along ?; same for u.
@@ -72,6 +73,7 @@ __device__ __forceinline__ V3<T> director_rhs(const FdConst<T>& C, V3<T> m, V3<T
   const V3<T> lap = ((mxp + mxm) + (myp + mym)) + (mzp + mzm) - T(6) * m;
   const V3<T> curl = {dym.z - dzm.y, dzm.x - dxm.z, dxm.y - dym.x};
   V3<T> R = C.inv_gamma1 * (C.K * lap - (T(2) * C.Kq0) * curl);
+  R.z += C.inv_gamma1 * (C.W0 * m.z);
   // velocity gradient G[b][c] = d_b u_c: rows dxu, dyu, dzu
   // (m.D)_mu = m_a D_{a mu} = 1/2 m_a (d_a u_mu + d_mu u_a)
   // (W.m)_mu = W_{mu a} m_a = 1/2 (d_a u_mu - d_mu u_a) m_a
@@ -160,7 +162,8 @@ __device__ __forceinline__ void viscous_add(const FdConst<T>& C, V3<T> n, V3<T> 
   const V3<T> Dx = {dxu.x, Dxy, Dxz}, Dy = {Dxy, dyu.y, Dyz}, Dz = {Dxz, Dyz, dzu.z};   // columns = rows
   const V3<T> nD = {dot(n, Dx), dot(n, Dy), dot(n, Dz)};
   const V3<T> curl = {dyn.z - dzn.y, dzn.x - dxn.z, dxn.y - dyn.x};
-  const V3<T> A = C.inv_gamma1 * (C.K * lap - (T(2) * C.Kq0) * curl) + C.xi * nD;
+  V3<T> A = C.inv_gamma1 * (C.K * lap - (T(2) * C.Kq0) * curl) + C.xi * nD;
+  A.z += C.inv_gamma1 * (C.W0 * n.z);
   const V3<T> N = A - dot(n, A) * n;
   const T nnD = dot(n, nD);
   const V3<T> w = C.al[1] * N + C.al[4] * nD;                  // multiplies n_b
@@ -238,6 +241,18 @@ store_director_kernel(const double* __restrict__ in, T* __restrict__ n, T* __res
   n[c] = (T)a; n[G.N + c] = (T)b; n[2 * G.N + c] = (T)d;
   nP[c] = (T)a; nP[G.N + c] = (T)b; nP[2 * G.N + c] = (T)d;
   nnew[c] = (T)a; nnew[G.N + c] = (T)b; nnew[2 * G.N + c] = (T)d;
+}
+
+// Free plates (anchoring = 1; reading G23): the plate layers copy the adjacent
+// fluid layer, so the stencils next to them see a zero normal derivative.  One thread per (c, y, x).
+template <typename T>
+__global__ void __launch_bounds__(256) mirror_plates_kernel(T* __restrict__ n, Geom G) {
+  const unsigned k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= 3u * G.plane) return;
+  const unsigned comp = k / G.plane, xy = k - comp * G.plane;
+  T* a = n + (size_t)comp * G.N + xy;
+  a[0] = a[G.plane];
+  a[(size_t)(G.nz - 1) * G.plane] = a[(size_t)(G.nz - 2) * G.plane];
 }
 
 __global__ void __launch_bounds__(256) fill_f64_kernel(double* __restrict__ p, double v, size_t n) {

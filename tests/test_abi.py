@@ -44,7 +44,7 @@ def test_workspace_bytes_and_validation(lib):
     p64 = nh.make_params(16, 16, 8, 0.8, precision=nh.FP64_SHIFTED)
     assert nh.workspace_bytes(p64) >= (2 * 19 + 6 * 3) * N * 8 + 3 * N * 8 + ring * 8
     for bad in (dict(tau=0.5), dict(nz=2), dict(gamma1=0.0), dict(K=-1.0), dict(fd_ratio=-1),
-                dict(W0=0.1), dict(precision=7), dict(anchoring=1), dict(nx=0), dict(coupling=4),
+                dict(W0=float("inf")), dict(precision=7), dict(anchoring=2), dict(nx=0), dict(coupling=4),
                 dict(nx=4096, ny=4096, nz=64)):
         kw = dict(nx=4, ny=4, nz=5, tau=0.8)
         kw.update(bad)
