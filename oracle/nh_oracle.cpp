@@ -102,14 +102,106 @@ void molecular_field_cell(const Grid& G, double K, double q0, const double* m, i
   h[2] += G.W0 * m[2 * N + c0];
 }
 
+// ---- three-constant Frank energy, Eqs. 7-8; row f2, reading G24 ----------
+// Discrete energy density at a cell, every derivative the central difference of Eq. 13:
+//   f = K11/2 (div n)^2 + K22/2 (n.curl n + q0)^2 + K33/2 |b|^2,   b = (n.grad) n
+// (|n x curl n| = |(n.grad) n| for a unit vector).  Its derivatives
+//   pi_{b c} = df/d(d_b n_c) = K11 delta_bc div n + K22 T eps_{a b c} n_a + K33 n_b b_c,  T = n.curl n + q0
+//   df/dn_m  = K22 T (curl n)_m + K33 b_c d_m n_c
+// give h_m = -df/dn_m + d_b pi_{b m} (Eq. 10) and sigma^e_{a b} = -d_a n_c pi_{b c} (Eq. 6).
+bool any_K3(const double K3[3]) { return K3[0] != 0.0 || K3[1] != 0.0 || K3[2] != 0.0; }
+
+void frank3_cell(const Grid& G, const double K3[3], double q0, const double* n, int x, int y, int z,
+                 double pi[3][3], double dfdn[3], double* fdens) {
+  const size_t N = G.N();
+  const size_t c0 = G.at(x, y, z);
+  double dn[3][3];  // dn[b][c] = d_b n_c
+  for (int b = 0; b < 3; ++b)
+    for (int c = 0; c < 3; ++c) dn[b][c] = ddx(G, n, c, x, y, z, b);
+  const double nn[3] = {n[c0], n[N + c0], n[2 * N + c0]};
+  const double div = dn[0][0] + dn[1][1] + dn[2][2];
+  double curl[3], bb[3];
+  for (int m = 0; m < 3; ++m) {
+    curl[m] = 0.0;
+    bb[m] = 0.0;
+    for (int b = 0; b < 3; ++b) {
+      bb[m] += nn[b] * dn[b][m];
+      for (int c = 0; c < 3; ++c) curl[m] += levi_civita(m, b, c) * dn[b][c];
+    }
+  }
+  const double T = nn[0] * curl[0] + nn[1] * curl[1] + nn[2] * curl[2] + q0;
+  for (int b = 0; b < 3; ++b)
+    for (int c = 0; c < 3; ++c) {
+      double twist = 0.0;
+      for (int a = 0; a < 3; ++a) twist += levi_civita(a, b, c) * nn[a];
+      pi[b][c] = K3[0] * (b == c ? div : 0.0) + K3[1] * T * twist + K3[2] * nn[b] * bb[c];
+    }
+  for (int m = 0; m < 3; ++m) {
+    double bend = 0.0;
+    for (int c = 0; c < 3; ++c) bend += bb[c] * dn[m][c];
+    dfdn[m] = K3[1] * T * curl[m] + K3[2] * bend;
+  }
+  if (fdens)
+    *fdens = 0.5 * K3[0] * div * div + 0.5 * K3[1] * T * T +
+             0.5 * K3[2] * (bb[0] * bb[0] + bb[1] * bb[1] + bb[2] * bb[2]);
+}
+
+// pi [9][N] (index 3 b + c) and df/dn [3][N] on the computed layers.  On the plate layers the director
+// is uniform inside the solid (solid node values fixed), so grad n = 0 there:
+// pi = K22 q0 eps_{a b c} n_a, df/dn unused.
+void frank3_fields(const Grid& G, const double K3[3], double q0, const double* n, double* pi, double* dfdn) {
+  const size_t N = G.N();
+  std::memset(dfdn, 0, sizeof(double) * 3 * N);
+  for (int z = 0; z < G.nz; ++z) {
+    if (z >= G.z_lo() && z < G.z_hi()) continue;
+    for (int y = 0; y < G.ny; ++y)
+      for (int x = 0; x < G.nx; ++x) {
+        const size_t c0 = G.at(x, y, z);
+        for (int b = 0; b < 3; ++b)
+          for (int c = 0; c < 3; ++c) {
+            double twist = 0.0;
+            for (int a = 0; a < 3; ++a) twist += levi_civita(a, b, c) * n[a * N + c0];
+            pi[(3 * b + c) * N + c0] = K3[1] * q0 * twist;
+          }
+      }
+  }
+#pragma omp parallel for schedule(static)
+  for (int z = G.z_lo(); z < G.z_hi(); ++z)
+    for (int y = 0; y < G.ny; ++y)
+      for (int x = 0; x < G.nx; ++x) {
+        double p[3][3], d[3];
+        frank3_cell(G, K3, q0, n, x, y, z, p, d, nullptr);
+        const size_t c0 = G.at(x, y, z);
+        for (int b = 0; b < 3; ++b)
+          for (int c = 0; c < 3; ++c) pi[(3 * b + c) * N + c0] = p[b][c];
+        for (int m = 0; m < 3; ++m) dfdn[m * N + c0] = d[m];
+      }
+}
+
+// h_m = -df/dn_m + d_b pi_{b m} (+ the bulk anchoring term) at one cell, from the fields above.
+void frank3_h_cell(const Grid& G, const double* n, const double* pi, const double* dfdn, int x, int y, int z,
+                   double h[3]) {
+  const size_t N = G.N();
+  const size_t c0 = G.at(x, y, z);
+  for (int m = 0; m < 3; ++m) {
+    double s = -dfdn[m * N + c0];
+    for (int b = 0; b < 3; ++b) s += ddx(G, pi, 3 * b + m, x, y, z, b);
+    h[m] = s;
+  }
+  h[2] += G.W0 * n[2 * N + c0];
+}
+
 // Right-hand side of the director equation, Eq. 9, with xi = -gamma2/gamma1 (G4),
 // D and W exactly as printed in Eq. 5 (G5), then projected perpendicular to m (G3).
+// pi, dfdn: the three-constant fields of frank3_fields for this m, or null for the one-constant energy.
 void director_rhs_cell(const Grid& G, double K, double q0, double xi, double gamma1,
-                       const double* m, const double* u, int x, int y, int z, double R[3]) {
+                       const double* m, const double* u, int x, int y, int z, double R[3],
+                       const double* pi = nullptr, const double* dfdn = nullptr) {
   const size_t N = G.N();
   const size_t c0 = G.at(x, y, z);
   double h[3];
-  molecular_field_cell(G, K, q0, m, x, y, z, h);
+  if (pi) frank3_h_cell(G, m, pi, dfdn, x, y, z, h);
+  else molecular_field_cell(G, K, q0, m, x, y, z, h);
   double dm[3][3], du[3][3];  // d_b m_c, d_b u_c
   for (int b = 0; b < 3; ++b)
     for (int c = 0; c < 3; ++c) {
@@ -140,12 +232,21 @@ void director_rhs_cell(const Grid& G, double K, double q0, double xi, double gam
 // Elastic stress, Eq. 6 for the energy of G1:
 // sigma_ab = -d_a n_c * dE/d(d_b n_c) = -K d_a n_c d_b n_c - K q0 eps_{mu b c} n_mu d_a n_c.
 void elastic_stress_cell(const Grid& G, double K, double q0, const double* n, int x, int y, int z,
-                         double sig[3][3]) {
+                         double sig[3][3], const double* pi = nullptr) {
   const size_t N = G.N();
   const size_t c0 = G.at(x, y, z);
   double dn[3][3];
   for (int b = 0; b < 3; ++b)
     for (int c = 0; c < 3; ++c) dn[b][c] = ddx(G, n, c, x, y, z, b);
+  if (pi) {  // three constants: sigma_ab = -d_a n_c pi_{b c} (Eq. 6)
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b) {
+        double s = 0.0;
+        for (int c = 0; c < 3; ++c) s -= dn[a][c] * pi[(3 * b + c) * N + c0];
+        sig[a][b] = s;
+      }
+    return;
+  }
   const double nn[3] = {n[c0], n[N + c0], n[2 * N + c0]};
   for (int a = 0; a < 3; ++a)
     for (int b = 0; b < 3; ++b) {
@@ -158,7 +259,8 @@ void elastic_stress_cell(const Grid& G, double K, double q0, const double* n, in
     }
 }
 
-void elastic_stress_field(const Grid& G, double K, double q0, const double* n, double* sigma) {
+void elastic_stress_field(const Grid& G, double K, double q0, const double* n, double* sigma,
+                          const double* pi = nullptr) {
   const size_t N = G.N();
   std::memset(sigma, 0, sizeof(double) * 9 * N);  // sigma = 0 on the plate layers (G6)
 #pragma omp parallel for schedule(static)
@@ -166,7 +268,7 @@ void elastic_stress_field(const Grid& G, double K, double q0, const double* n, d
     for (int y = 0; y < G.ny; ++y)
       for (int x = 0; x < G.nx; ++x) {
         double s[3][3];
-        elastic_stress_cell(G, K, q0, n, x, y, z, s);
+        elastic_stress_cell(G, K, q0, n, x, y, z, s, pi);
         for (int a = 0; a < 3; ++a)
           for (int b = 0; b < 3; ++b) sigma[(3 * a + b) * N + G.at(x, y, z)] = s[a][b];
       }
@@ -198,7 +300,8 @@ void elastic_force_field(const Grid& G, double K, double q0, const double* n, do
 // perpendicular to n like the director's rate itself (reading G22), so no time derivative
 // is needed.
 void viscous_stress_cell(const Grid& G, double K, double q0, double xi, double gamma1, const double al[6],
-                         const double* n, const double* u, int x, int y, int z, double sig[3][3]) {
+                         const double* n, const double* u, int x, int y, int z, double sig[3][3],
+                         const double* pi = nullptr, const double* dfdn = nullptr) {
   const size_t N = G.N();
   const size_t c0 = G.at(x, y, z);
   double du[3][3];  // d_b u_c
@@ -209,7 +312,8 @@ void viscous_stress_cell(const Grid& G, double K, double q0, double xi, double g
     for (int b = 0; b < 3; ++b) D[a][b] = 0.5 * (du[a][b] + du[b][a]);
   const double nn[3] = {n[c0], n[N + c0], n[2 * N + c0]};
   double h[3];
-  molecular_field_cell(G, K, q0, n, x, y, z, h);
+  if (pi) frank3_h_cell(G, n, pi, dfdn, x, y, z, h);
+  else molecular_field_cell(G, K, q0, n, x, y, z, h);
   double nD[3], A[3];  // nD_b = n_m D_mb
   for (int b = 0; b < 3; ++b) {
     nD[b] = 0.0;
@@ -235,14 +339,15 @@ bool any_alpha(const double al[6]) {
 
 // sigma (+)= sigma^v on the computed layers; the plate layers stay 0 (G6).
 void viscous_stress_add(const Grid& G, double K, double q0, double xi, double gamma1, const double al[6],
-                        const double* n, const double* u, double* sigma) {
+                        const double* n, const double* u, double* sigma,
+                        const double* pi = nullptr, const double* dfdn = nullptr) {
   const size_t N = G.N();
 #pragma omp parallel for schedule(static)
   for (int z = G.z_lo(); z < G.z_hi(); ++z)
     for (int y = 0; y < G.ny; ++y)
       for (int x = 0; x < G.nx; ++x) {
         double s[3][3];
-        viscous_stress_cell(G, K, q0, xi, gamma1, al, n, u, x, y, z, s);
+        viscous_stress_cell(G, K, q0, xi, gamma1, al, n, u, x, y, z, s, pi, dfdn);
         for (int a = 0; a < 3; ++a)
           for (int b = 0; b < 3; ++b) sigma[(3 * a + b) * N + G.at(x, y, z)] += s[a][b];
       }
@@ -250,11 +355,22 @@ void viscous_stress_add(const Grid& G, double K, double q0, double xi, double ga
 
 // F^LC_a = d_b (sigma^e_ab + sigma^v_ab) by central differences: Eq. 12.
 void lc_force_field(const Grid& G, double K, double q0, double xi, double gamma1, const double al[6],
-                    const double* n, const double* u, double* F, std::vector<double>& sigma) {
+                    const double* n, const double* u, double* F, std::vector<double>& sigma,
+                    const double* K3 = nullptr) {
   const size_t N = G.N();
   sigma.resize(9 * N);
-  elastic_stress_field(G, K, q0, n, sigma.data());
-  if (any_alpha(al)) viscous_stress_add(G, K, q0, xi, gamma1, al, n, u, sigma.data());
+  std::vector<double> pi, dfdn;
+  const double* ppi = nullptr;
+  const double* pdf = nullptr;
+  if (K3 && any_K3(K3)) {
+    pi.resize(9 * N);
+    dfdn.resize(3 * N);
+    frank3_fields(G, K3, q0, n, pi.data(), dfdn.data());
+    ppi = pi.data();
+    pdf = dfdn.data();
+  }
+  elastic_stress_field(G, K, q0, n, sigma.data(), ppi);
+  if (any_alpha(al)) viscous_stress_add(G, K, q0, xi, gamma1, al, n, u, sigma.data(), ppi, pdf);
   std::memset(F, 0, sizeof(double) * 3 * N);
 #pragma omp parallel for schedule(static)
   for (int z = G.z_lo(); z < G.z_hi(); ++z)
@@ -268,15 +384,25 @@ void lc_force_field(const Grid& G, double K, double q0, double xi, double gamma1
 }
 
 void director_rhs_field(const Grid& G, double K, double q0, double xi, double gamma1,
-                        const double* m, const double* u, double* R) {
+                        const double* m, const double* u, double* R, const double* K3 = nullptr) {
   const size_t N = G.N();
   std::memset(R, 0, sizeof(double) * 3 * N);
+  std::vector<double> pi, dfdn;
+  const double* ppi = nullptr;
+  const double* pdf = nullptr;
+  if (K3 && any_K3(K3)) {
+    pi.resize(9 * N);
+    dfdn.resize(3 * N);
+    frank3_fields(G, K3, q0, m, pi.data(), dfdn.data());
+    ppi = pi.data();
+    pdf = dfdn.data();
+  }
 #pragma omp parallel for schedule(static)
   for (int z = G.z_lo(); z < G.z_hi(); ++z)
     for (int y = 0; y < G.ny; ++y)
       for (int x = 0; x < G.nx; ++x) {
         double r[3];
-        director_rhs_cell(G, K, q0, xi, gamma1, m, u, x, y, z, r);
+        director_rhs_cell(G, K, q0, xi, gamma1, m, u, x, y, z, r, ppi, pdf);
         for (int c = 0; c < 3; ++c) R[c * N + G.at(x, y, z)] = r[c];
       }
 }
@@ -414,7 +540,7 @@ struct nh_oracle_lattice {
     if (any_alpha(p.alpha)) {
       if (!have_u) { uv.resize(3 * G.N()); velocity_field(nullptr, uv.data()); uu = uv.data(); }
     }
-    lc_force_field(G, p.K, q0, p.xi, p.gamma1, p.alpha, n.data(), uu, F.data(), sigma);
+    lc_force_field(G, p.K, q0, p.xi, p.gamma1, p.alpha, n.data(), uu, F.data(), sigma, p.K3);
   }
 
   // FD update with Delta t_FD = r, same u for both stages (G11).
@@ -423,9 +549,9 @@ struct nh_oracle_lattice {
     if (p.coupling & 2) velocity_field(nullptr, u.data());
     else std::fill(u.begin(), u.end(), 0.0);
     const double dt = (double)r;
-    director_rhs_field(G, p.K, q0, p.xi, p.gamma1, n.data(), u.data(), k1.data());   // (d_t n)_old
+    director_rhs_field(G, p.K, q0, p.xi, p.gamma1, n.data(), u.data(), k1.data(), p.K3);   // (d_t n)_old
     normalise_into(nP, n, k1, nullptr, dt);                                          // predictor
-    director_rhs_field(G, p.K, q0, p.xi, p.gamma1, nP.data(), u.data(), k2.data());  // (d_t n)_P
+    director_rhs_field(G, p.K, q0, p.xi, p.gamma1, nP.data(), u.data(), k2.data(), p.K3);  // (d_t n)_P
     normalise_into(nnew, n, k1, &k2, dt);                                            // corrector
     n.swap(nnew);
     lc_force(/*have_u=*/(p.coupling & 2) != 0);                                     // Eq. 12
@@ -451,6 +577,8 @@ int nh_oracle_init_lattice(const nh_oracle_params* p, nh_oracle_lattice** out) {
   if (!(p->tau > 0.5)) return fail(E_INVAL, "tau must be > 0.5");
   if (!(p->gamma1 > 0.0)) return fail(E_INVAL, "gamma1 must be > 0");
   if (p->K < 0.0) return fail(E_INVAL, "K must be >= 0");
+  for (int i = 0; i < 3; ++i)
+    if (!(p->K3[i] >= 0.0)) return fail(E_INVAL, "K11, K22, K33 must be >= 0");
   if (p->fd_ratio < 0) return fail(E_INVAL, "fd_ratio must be >= 0");
   if (p->precision < 0 || p->precision > 3) return fail(E_INVAL, "precision must be 0..3");
   if (p->anchoring != 0 && p->anchoring != 1) return fail(E_INVAL, "anchoring must be 0 (homeotropic plates) or 1 (free plates)");
@@ -627,6 +755,40 @@ int nh_oracle_elastic_force(int nx, int ny, int nz, int periodic_z, double K, do
   const Grid G{nx, ny, nz, periodic_z != 0};
   std::vector<double> sigma;
   elastic_force_field(G, K, q0, n, F, sigma);
+  return 0;
+}
+
+/* three-constant energy (row f2): K3 = {K11, K22, K33}; E = sum of f over the computed layers */
+int nh_oracle_frank3(int nx, int ny, int nz, int periodic_z, const double* K3, double q0, const double* n,
+                     double* h, double* sigma, double* energy) {
+  if (!n || !K3 || bad_dims(nx, ny, nz)) return fail(E_INVAL, "bad arguments");
+  const Grid G{nx, ny, nz, periodic_z != 0};
+  const size_t N = G.N();
+  std::vector<double> pi(9 * N), dfdn(3 * N);
+  frank3_fields(G, K3, q0, n, pi.data(), dfdn.data());
+  if (h) std::memset(h, 0, sizeof(double) * 3 * N);
+  if (sigma) std::memset(sigma, 0, sizeof(double) * 9 * N);
+  double E = 0.0;
+  for (int z = G.z_lo(); z < G.z_hi(); ++z)
+    for (int y = 0; y < ny; ++y)
+      for (int x = 0; x < nx; ++x) {
+        const size_t c0 = G.at(x, y, z);
+        if (h) {
+          double hh[3];
+          frank3_h_cell(G, n, pi.data(), dfdn.data(), x, y, z, hh);
+          for (int c = 0; c < 3; ++c) h[c * N + c0] = hh[c];
+        }
+        if (sigma) {
+          double s[3][3];
+          elastic_stress_cell(G, 0.0, q0, n, x, y, z, s, pi.data());
+          for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) sigma[(3 * a + b) * N + c0] = s[a][b];
+        }
+        double p[3][3], d[3], f;
+        frank3_cell(G, K3, q0, n, x, y, z, p, d, &f);
+        E += f;
+      }
+  if (energy) *energy = E;
   return 0;
 }
 

@@ -59,6 +59,9 @@ typedef struct {
   double alpha[6];     /* Leslie viscosities alpha1, alpha2, alpha3, alpha4', alpha5, alpha6 of the
                           viscous stress in the force, Eqs. 3, 12; all 0 = elastic stress only
                                                                          PAPER.md:50, 97-99 */
+  double K3[3];        /* K11, K22, K33 of Eqs. 7-8 (splay, twist, bend); all 0 = the one-constant
+                          energy with K; otherwise K is ignored (row f2, reading G24)
+                                                                         PAPER.md:70-73   */
 } nh_oracle_params;
 
 int  nh_oracle_init_lattice(const nh_oracle_params*, nh_oracle_lattice** out);
@@ -87,6 +90,10 @@ int nh_oracle_elastic_stress(int nx, int ny, int nz, int periodic_z, double K, d
                              const double* n, double* sigma /* [9][nz][ny][nx], index 3*alpha+beta */);
 int nh_oracle_elastic_force(int nx, int ny, int nz, int periodic_z, double K, double q0,
                             const double* n, double* F);
+/* Three-constant Frank energy (Eqs. 7-8), K3 = {K11, K22, K33}: molecular field h [3][N], elastic
+ * stress sigma [9][N] and the total discrete energy; any output pointer may be NULL. */
+int nh_oracle_frank3(int nx, int ny, int nz, int periodic_z, const double* K3, double q0, const double* n,
+                     double* h, double* sigma, double* energy);
 /* Leslie viscous stress of Eq. 3 with alpha4 -> alpha4' (Eq. 12), N from Eq. 9 (reading G22), and
  * the whole force F^LC = d_b (sigma^e + sigma^v)_ab.  alpha = {a1, a2, a3, a4', a5, a6}. */
 int nh_oracle_viscous_stress(int nx, int ny, int nz, int periodic_z, double K, double q0, double xi,

@@ -12,7 +12,8 @@ class _Params(C.Structure):
                 ("tau", C.c_double), ("K", C.c_double), ("pitch", C.c_double),
                 ("xi", C.c_double), ("gamma1", C.c_double), ("g", C.c_double * 3),
                 ("anchoring", C.c_int), ("W0", C.c_double), ("fd_ratio", C.c_int),
-                ("precision", C.c_int), ("coupling", C.c_int), ("alpha", C.c_double * 6)]
+                ("precision", C.c_int), ("coupling", C.c_int), ("alpha", C.c_double * 6),
+                ("K3", C.c_double * 3)]
 
 
 class OracleError(RuntimeError):
@@ -43,6 +44,7 @@ def _load():
         lib.nh_oracle_director_rhs.argtypes = [C.c_int] * 4 + [C.c_double] * 4 + [dp, dp, dp]
         lib.nh_oracle_elastic_stress.argtypes = [C.c_int] * 4 + [C.c_double] * 2 + [dp, dp]
         lib.nh_oracle_elastic_force.argtypes = [C.c_int] * 4 + [C.c_double] * 2 + [dp, dp]
+        lib.nh_oracle_frank3.argtypes = [C.c_int] * 4 + [dp, C.c_double, dp, dp, dp, dp]
         lib.nh_oracle_viscous_stress.argtypes = [C.c_int] * 4 + [C.c_double] * 4 + [dp, dp, dp, dp]
         lib.nh_oracle_lc_force.argtypes = [C.c_int] * 4 + [C.c_double] * 4 + [dp, dp, dp, dp]
         _lib = lib
@@ -73,10 +75,10 @@ class Oracle:
     """One oracle lattice; same call surface as the CUDA binding (init / set_director / step / get_fields)."""
 
     def __init__(self, nx, ny, nz, tau, K=0.0, pitch=0.0, xi=0.0, gamma1=1.0, g=(0.0, 0.0, 0.0),
-                 anchoring=0, W0=0.0, fd_ratio=1, precision=0, coupling=3, alpha=(0.0,) * 6, **_ignored):
+                 anchoring=0, W0=0.0, fd_ratio=1, precision=0, coupling=3, alpha=(0.0,) * 6, K3=(0.0, 0.0, 0.0), **_ignored):
         lib = _load()
         self.p = _Params(nx, ny, nz, tau, K, pitch, xi, gamma1, (C.c_double * 3)(*g), anchoring, W0,
-                         fd_ratio, precision, coupling, (C.c_double * 6)(*alpha))
+                         fd_ratio, precision, coupling, (C.c_double * 6)(*alpha), (C.c_double * 3)(*K3))
         self.shape = (nz, ny, nx)
         self._h = C.c_void_p()
         _check(lib.nh_oracle_init_lattice(C.byref(self.p), C.byref(self._h)))
@@ -180,3 +182,16 @@ def lc_force(n, u, K, q0, xi, gamma1, alpha, periodic_z=False):
     _check(_load().nh_oracle_lc_force(nx, ny, nz, int(periodic_z), K, q0, xi, gamma1, _ptr(al),
                                       _ptr(n), _ptr(u), _ptr(F)))
     return F
+
+
+def frank3(n, K3, q0, periodic_z=False):
+    """Three-constant Frank energy (Eqs. 7-8): returns (h [3,...], sigma [3,3,...], total energy)."""
+    n = np.ascontiguousarray(n, dtype=np.float64)
+    k3 = np.ascontiguousarray(K3, dtype=np.float64)
+    nx, ny, nz = _dims(n)
+    h = np.empty_like(n)
+    s = np.empty((9, nz, ny, nx))
+    e = C.c_double(0.0)
+    _check(_load().nh_oracle_frank3(nx, ny, nz, int(periodic_z), _ptr(k3), q0, _ptr(n), _ptr(h), _ptr(s),
+                                    C.cast(C.byref(e), C.POINTER(C.c_double))))
+    return h, s.reshape(3, 3, nz, ny, nx), e.value
