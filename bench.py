@@ -45,6 +45,8 @@ def parse():
     ap.add_argument("--block-order", action="store_true", help="NH_OPT_LB_BLOCKORDER: two-step units in blockIdx order")
     ap.add_argument("--leslie", type=float, default=0.0,
                     help="scale of the paper's Table-1 Leslie viscosities in the force (row f1; 0 = elastic stress only)")
+    ap.add_argument("--frank3", action="store_true",
+                    help="three-constant Frank energy (row f2): K11 = K, K22 : K33 in the ratios of the paper's Table 1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -60,6 +62,9 @@ def workload(args):
         # alpha1..alpha6 of MBBA in simulation units as printed in the paper's Table 1
         table1 = (0.0373, -0.4496, -0.0203, 0.9318, 0.3084, -0.1617)
         p["alpha"] = tuple(args.leslie * a for a in table1)
+    if args.frank3:
+        # K11 : K22 : K33 = 1.67 : 0.788 : 2.62
+        p["K3"] = (p["K"], p["K"] * 0.788 / 1.67, p["K"] * 2.62 / 1.67)
     d = p.pop("director")
     p.pop("steps")
     name = {0: "configs[0] tiny channel", 1: "configs[1] single skyrmion tube", 2: "configs[2] precision sweep domain",
@@ -69,6 +74,8 @@ def workload(args):
             "g_x": p["g"][0], "precision": args.precision}
     if args.leslie:
         desc["leslie_viscous_stress"] = "Table 1 x %g" % args.leslie
+    if args.frank3:
+        desc["frank_constants"] = list(p["K3"])
     return p, d, desc
 
 

@@ -74,6 +74,10 @@ typedef struct {
                           All 0 (the north_star's reduced model): elastic stress only.  xi and gamma1 are
                           NOT derived from them (gamma1 = alpha3 - alpha2, gamma2 = alpha3 + alpha2 is
                           the caller's business) */
+  double K3[3];        /* K11, K22, K33 (splay, twist, bend) of the Frank energy, Eqs. 7-8; all 0: the
+                          one-constant energy with K (the north_star's model); otherwise K is ignored
+                          and h, sigma^e follow from the three-constant energy (G24)
+                                                                                  PAPER.md:70-73 */
 } nh_params;
 
 /* Bytes of device memory the lattice needs for these parameters (0 if they are invalid).

@@ -28,7 +28,8 @@ class NhParams(C.Structure):
                 ("tau", C.c_double), ("K", C.c_double), ("pitch", C.c_double),
                 ("xi", C.c_double), ("gamma1", C.c_double), ("g", C.c_double * 3),
                 ("anchoring", C.c_int), ("W0", C.c_double), ("fd_ratio", C.c_int),
-                ("precision", C.c_int), ("coupling", C.c_int), ("alpha", C.c_double * 6)]
+                ("precision", C.c_int), ("coupling", C.c_int), ("alpha", C.c_double * 6),
+                ("K3", C.c_double * 3)]
 
 
 class NhError(RuntimeError):
@@ -75,9 +76,9 @@ def _check(rc):
 
 
 def make_params(nx, ny, nz, tau, K=0.0, pitch=0.0, xi=0.0, gamma1=1.0, g=(0.0, 0.0, 0.0), anchoring=0,
-                W0=0.0, fd_ratio=1, precision=FP32_SHIFTED, coupling=3, alpha=(0.0,) * 6) -> NhParams:
+                W0=0.0, fd_ratio=1, precision=FP32_SHIFTED, coupling=3, alpha=(0.0,) * 6, K3=(0.0, 0.0, 0.0)) -> NhParams:
     return NhParams(nx, ny, nz, tau, K, pitch, xi, gamma1, (C.c_double * 3)(*g), anchoring, W0,
-                    fd_ratio, precision, coupling, (C.c_double * 6)(*alpha))
+                    fd_ratio, precision, coupling, (C.c_double * 6)(*alpha), (C.c_double * 3)(*K3))
 
 
 def workspace_bytes(params: NhParams) -> int:

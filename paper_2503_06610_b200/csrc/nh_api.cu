@@ -15,6 +15,7 @@
 
 #include "nh_fd.cuh"
 #include "nh_fd_tile.cuh"
+#include "nh_frank3.cuh"
 #include "nh_lb.cuh"
 #include "nh_lb2.cuh"
 #include "nh_lb_vec.cuh"
@@ -52,8 +53,11 @@ const char* check_params(const nh_params* p) {
   if (!std::isfinite(p->W0)) return "W0 must be finite";
   if (p->coupling < 0 || p->coupling > 3) return "coupling must be 0..3";
   for (int i = 0; i < 6; ++i) if (!std::isfinite(p->alpha[i])) return "alpha must be finite";
+  for (int i = 0; i < 3; ++i) if (!(p->K3[i] >= 0.0) || !std::isfinite(p->K3[i])) return "K11, K22, K33 must be >= 0";
   return nullptr;
 }
+
+bool three_constants(const nh_params* p) { return p->K3[0] != 0.0 || p->K3[1] != 0.0 || p->K3[2] != 0.0; }
 
 size_t word_of(int precision) {
   return (precision == NH_FP64_SHIFTED || precision == NH_FP64_UNSHIFTED) ? 8 : 4;
@@ -88,6 +92,9 @@ struct nh_lattice {
   void* a;          // n + dt/2 k1, predictor -> corrector (tiled FD kernels)
   void* u;
   void* F;
+  void* pi3;        // three-constant energy only: pi [9][N], df/dn [3][N], h [3][N]
+  void* dfdn3;
+  void* h3;
   double* stage;    // FP64 staging [3][N]
   int* flag;
   int sweep;        // direction of the next population sweep (alternates, see sweep_block)
@@ -363,6 +370,30 @@ bool tiles_fit(const nh_lattice* L) {
   return g.grid.y <= 65535u && g.grid.z <= 65535u;
 }
 
+// ---- three-constant Frank energy (nh_frank3.cuh) ------------------------------------------------
+template <typename T>
+nh::Frank3<T> frank3_const(const nh_lattice* L) {
+  nh::Frank3<T> K;
+  K.K11 = (T)L->p.K3[0]; K.K22 = (T)L->p.K3[1]; K.K33 = (T)L->p.K3[2]; K.q0 = (T)L->q0;
+  return K;
+}
+// h[m] of the three-constant energy into L->h3 (pi and df/dn stay in their buffers for the stress)
+template <typename T>
+int launch_h3(nh_lattice* L, const void* m, int cls) {
+  {
+    Bracket br(L, cls);
+    if (br.rc) return br.rc;
+    nh::pi3_kernel<T><<<blocks_for(L->G.N), BLOCK, 0, L->stream>>>((const T*)m, (T*)L->pi3, (T*)L->dfdn3, L->G, frank3_const<T>(L));
+    br.end();
+  }
+  Bracket br(L, cls);
+  if (br.rc) return br.rc;
+  nh::h3_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>((const T*)m, (const T*)L->pi3, (const T*)L->dfdn3,
+                                                                    (T*)L->h3, L->G, (T)L->p.W0);
+  br.end();
+  return NH_OK;
+}
+
 bool viscous(const nh_lattice* L) {
   for (int i = 0; i < 6; ++i) if (L->p.alpha[i] != 0.0) return true;
   return false;
@@ -376,6 +407,16 @@ int launch_force(nh_lattice* L) {
   const nh::FdConst<T> C = fd_const<T>(L, 1);
   const T* n = (const T*)L->n[L->ncur];
   const T* u = (const T*)L->u;
+  if (three_constants(&L->p)) {
+    br.end();
+    { const int rc = launch_h3<T>(L, n, KC_FORCE); if (rc) return rc; }
+    Bracket b3(L, KC_FORCE);
+    if (b3.rc) return b3.rc;
+    nh::force3_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(n, u, (const T*)L->pi3, (const T*)L->h3,
+                                                                          (T*)L->F, L->G, C);
+    b3.end();
+    return NH_OK;
+  }
   if (!(L->options & NH_OPT_FD_DIRECT) && tiles_fit(L)) {
     const TileGrid g = tile_grid(L);
     const bool vec = tiles_vec(L);
@@ -411,6 +452,30 @@ int launch_director(nh_lattice* L, int r) {
   const nh::FdConst<T> C = fd_const<T>(L, r);
   const bool tiled = !(L->options & NH_OPT_FD_DIRECT) && tiles_fit(L);
   const TileGrid g = tile_grid(L);
+  if (three_constants(&L->p)) {
+    int rc = launch_h3<T>(L, L->n[L->ncur], KC_PRED);
+    if (rc) return rc;
+    {
+      Bracket br(L, KC_PRED);
+      if (br.rc) return br.rc;
+      nh::rhs3_kernel<T, 0><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
+          (const T*)L->n[L->ncur], (const T*)L->u, (const T*)L->h3, nullptr, (T*)L->nP, (T*)L->a, L->G, C, with_flow);
+      br.end();
+    }
+    rc = mirror_plates<T>(L, L->nP);
+    if (rc) return rc;
+    rc = launch_h3<T>(L, L->nP, KC_CORR);
+    if (rc) return rc;
+    {
+      Bracket br(L, KC_CORR);
+      if (br.rc) return br.rc;
+      nh::rhs3_kernel<T, 1><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(
+          (const T*)L->nP, (const T*)L->u, (const T*)L->h3, (const T*)L->a, (T*)L->n[L->ncur ^ 1], nullptr, L->G, C, with_flow);
+      br.end();
+    }
+    L->ncur ^= 1;
+    return mirror_plates<T>(L, L->n[L->ncur]);
+  }
   {
     Bracket br(L, KC_PRED);
     if (br.rc) return br.rc;
@@ -648,6 +713,7 @@ size_t nh_workspace_bytes(const nh_params* p) {
   b += 6 * align_up(3 * N * w);    // n[0], n[1], nP, a, u, F
   b += align_up(3 * N * sizeof(double));  // staging
   b += ALIGN;                      // flag
+  if (three_constants(p)) b += align_up(9 * N * w) + 2 * align_up(3 * N * w);   // pi, df/dn, h
   b += align_up((size_t)ring_planes(p) * 19 * p->nx * p->ny * w);   // plane ring of the two-step LB kernel
   b += align_up(wave_words(p) * 8);                                 // its counters
   return b;
@@ -686,6 +752,8 @@ int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_strea
   L->nP = take(3 * N * w); L->a = take(3 * N * w); L->u = take(3 * N * w); L->F = take(3 * N * w);
   L->stage = (double*)take(3 * N * sizeof(double));
   L->flag = (int*)take(sizeof(int));
+  L->pi3 = L->dfdn3 = L->h3 = nullptr;
+  if (three_constants(p)) { L->pi3 = take(9 * N * w); L->dfdn3 = take(3 * N * w); L->h3 = take(3 * N * w); }
   L->ring_cap = ring_planes(p);
   L->ring = take((size_t)L->ring_cap * 19 * L->G.plane * w);
   L->wave = (unsigned long long*)take(wave_words(p) * 8);

@@ -59,6 +59,10 @@ __device__ __forceinline__ Nbr neighbours(const Geom& G, int x, int y, int z) {
   return b;
 }
 
+template <typename T>
+__device__ __forceinline__ V3<T> director_rhs_tail(const FdConst<T>& C, V3<T> R, V3<T> m, V3<T> dxm, V3<T> dym,
+                                                   V3<T> dzm, V3<T> u, V3<T> dxu, V3<T> dyu, V3<T> dzu);
+
 // Right-hand side of Eq. 9 at one cell from the centre value and the six neighbours of m and u.
 //   h   = K lap m - 2 K q0 curl m + W0 m_z z_hat   (7-point Laplacian, central curl; bulk anchoring)
 //   R   = h/gamma1 + xi m.D - (u.grad) m + W.m,   D, W as printed in Eq. 5
@@ -74,6 +78,14 @@ __device__ __forceinline__ V3<T> director_rhs(const FdConst<T>& C, V3<T> m, V3<T
   const V3<T> curl = {dym.z - dzm.y, dzm.x - dxm.z, dxm.y - dym.x};
   V3<T> R = C.inv_gamma1 * (C.K * lap - (T(2) * C.Kq0) * curl);
   R.z += C.inv_gamma1 * (C.W0 * m.z);
+  return director_rhs_tail(C, R, m, dxm, dym, dzm, u, dxu, dyu, dzu);
+}
+
+// The same from a given h/gamma1 (three-constant energy, nh_frank3.cuh): flow terms and projection.
+template <typename T>
+__device__ __forceinline__ V3<T> director_rhs_tail(const FdConst<T>& C, V3<T> R, V3<T> m, V3<T> dxm, V3<T> dym,
+                                                   V3<T> dzm, V3<T> u, V3<T> dxu, V3<T> dyu, V3<T> dzu) {
+  const T h = T(0.5);
   // velocity gradient G[b][c] = d_b u_c: rows dxu, dyu, dzu
   // (m.D)_mu = m_a D_{a mu} = 1/2 m_a (d_a u_mu + d_mu u_a)
   // (W.m)_mu = W_{mu a} m_a = 1/2 (d_a u_mu - d_mu u_a) m_a
@@ -147,6 +159,10 @@ __device__ __forceinline__ V3<T> stress_column(const FdConst<T>& C, int b, V3<T>
   return {C.Kq0 * qx - C.K * dot(dxn, db), C.Kq0 * qy - C.K * dot(dyn, db), C.Kq0 * qz - C.K * dot(dzn, db)};
 }
 
+template <typename T>
+__device__ __forceinline__ void viscous_add_h(const FdConst<T>& C, V3<T> n, V3<T> hg, V3<T> dxu, V3<T> dyu,
+                                              V3<T> dzu, V3<T>& sx, V3<T>& sy, V3<T>& sz);
+
 // Leslie viscous stress, Eq. 3 with alpha4 -> alpha4' as in the force of Eq. 12
 // (PAPER.md:97-99), added column by column: s?[a] += sigma^v_{a ?},
 //   sigma^v_ab = a1 n_a n_b (n.D.n) + a2 n_b N_a + a3 n_a N_b + a4' D_ab + a5 n_b (n.D)_a + a6 n_a (n.D)_b
@@ -157,13 +173,21 @@ template <typename T>
 __device__ __forceinline__ void viscous_add(const FdConst<T>& C, V3<T> n, V3<T> dxn, V3<T> dyn, V3<T> dzn,
                                             V3<T> lap, V3<T> dxu, V3<T> dyu, V3<T> dzu,
                                             V3<T>& sx, V3<T>& sy, V3<T>& sz) {
+  const V3<T> curl = {dyn.z - dzn.y, dzn.x - dxn.z, dxn.y - dyn.x};
+  V3<T> hg = C.inv_gamma1 * (C.K * lap - (T(2) * C.Kq0) * curl);
+  hg.z += C.inv_gamma1 * (C.W0 * n.z);
+  viscous_add_h(C, n, hg, dxu, dyu, dzu, sx, sy, sz);
+}
+
+// The same from a given h/gamma1 (any energy).
+template <typename T>
+__device__ __forceinline__ void viscous_add_h(const FdConst<T>& C, V3<T> n, V3<T> hg, V3<T> dxu, V3<T> dyu,
+                                              V3<T> dzu, V3<T>& sx, V3<T>& sy, V3<T>& sz) {
   const T h2 = T(0.5);
   const T Dxy = h2 * (dxu.y + dyu.x), Dxz = h2 * (dxu.z + dzu.x), Dyz = h2 * (dyu.z + dzu.y);
   const V3<T> Dx = {dxu.x, Dxy, Dxz}, Dy = {Dxy, dyu.y, Dyz}, Dz = {Dxz, Dyz, dzu.z};   // columns = rows
   const V3<T> nD = {dot(n, Dx), dot(n, Dy), dot(n, Dz)};
-  const V3<T> curl = {dyn.z - dzn.y, dzn.x - dxn.z, dxn.y - dyn.x};
-  V3<T> A = C.inv_gamma1 * (C.K * lap - (T(2) * C.Kq0) * curl) + C.xi * nD;
-  A.z += C.inv_gamma1 * (C.W0 * n.z);
+  const V3<T> A = hg + C.xi * nD;
   const V3<T> N = A - dot(n, A) * n;
   const T nnD = dot(n, nD);
   const V3<T> w = C.al[1] * N + C.al[4] * nD;                  // multiplies n_b
