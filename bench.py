@@ -45,6 +45,7 @@ def parse():
     ap.add_argument("--block-order", action="store_true", help="NH_OPT_LB_BLOCKORDER: two-step units in blockIdx order")
     ap.add_argument("--leslie", type=float, default=0.0,
                     help="scale of the paper's Table-1 Leslie viscosities in the force (row f1; 0 = elastic stress only)")
+    ap.add_argument("--fd-ratio", type=int, default=None, help="override the config's Delta t_FD / Delta t_LB")
     ap.add_argument("--frank3", action="store_true",
                     help="three-constant Frank energy (row f2): K11 = K, K22 : K33 in the ratios of the paper's Table 1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -57,6 +58,8 @@ def workload(args):
     over = {}
     if args.config == 4 and args.size:
         over["size"] = tuple(args.size)
+    if args.fd_ratio is not None:
+        over["fd_ratio"] = args.fd_ratio
     p = I.config(args.config, **over)
     if args.leslie:
         # alpha1..alpha6 of MBBA in simulation units as printed in the paper's Table 1
