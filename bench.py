@@ -92,21 +92,22 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic(precision_name, grid):
+def ncu_traffic(precision_name, grid, with_inst=False):
     """DRAM bytes per LB launch from the committed ncu --set full capture (profiles/lb_traffic.csv), or None."""
     path = os.path.join(ROOT, "profiles", "lb_traffic.csv")
     if not os.path.exists(path):
-        return None
+        return (None, None) if with_inst else None
     try:
         want = "%dx%dx%d" % tuple(grid)
-        val = None
+        val = inst = None
         for line in open(path).read().splitlines()[1:]:
             c = line.split(",")
             if len(c) >= 4 and c[0] == precision_name and c[1] == want:
                 val = float(c[3])     # the last matching row is the newest capture
-        return val
+                inst = float(c[5]) if len(c) >= 6 and c[5] else None
+        return (val, inst) if with_inst else val
     except Exception:
-        return None
+        return (None, None) if with_inst else None
 
 
 class ClockSampler:
@@ -317,6 +318,12 @@ def main():
         # what the DRAM actually moved (ncu capture of the same kernel) over the live launch time
         roofline["dram_gbs"] = roofline["traffic"] / (lb_avg * 1e-3) / 1e9
         roofline["dram_frac"] = roofline["dram_gbs"] / peak
+    inst = ncu_traffic(args.precision + ("+2step" if two else ""), desc["grid"], with_inst=True)[1]
+    if inst and lb_avg > 0 and clocks and clocks.get("sm_mhz"):
+        # second ceiling: warp instructions issued against 148 SMs x 4 issue slots per clock
+        issue_peak = 148 * 4 * clocks["sm_mhz"] * 1e6
+        roofline["issue_frac"] = inst / (lb_avg * 1e-3) / issue_peak
+        roofline["warp_instructions_per_launch"] = inst
     if two:
         roofline["note"] = ("two LB steps share one pass over HBM (the intermediate step lives in an L2-resident "
                             "plane ring), so the algorithmic bytes of two steps move in about the DRAM traffic of "
