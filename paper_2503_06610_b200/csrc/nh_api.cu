@@ -69,8 +69,8 @@ enum KernelClass { KC_LB = 0, KC_VEL = 1, KC_PRED = 2, KC_CORR = 3, KC_FORCE = 4
 int ring_planes(const nh_params* p) { return p->nz - 2 < 12 ? p->nz - 2 : 12; }
 // u64 words of the two-step kernel's control block: 8 header words, then two u32 flags per plane and piece
 size_t wave_words(const nh_params* p) {
-  const size_t pieces = (size_t)p->nx * p->ny / 128 + p->ny + 1;   // upper bound over the piece shapes
-  return 8 + (size_t)(p->nz - 2) * pieces + (size_t)(p->nz - 2) + 8;   // + the launch-order table
+  const size_t pieces = (size_t)p->nx * (p->ny + 2) / 128 + p->ny + 3;   // = lb2_max_pieces: bound over the piece shapes
+  return 8 + 32 + (size_t)(p->nz - 2) * pieces + (size_t)(p->nz - 2) + 8;   // header, strip counters, flags, order table
 }
 
 }  // namespace
@@ -102,6 +102,7 @@ struct nh_lattice {
   int ring_cap;     // planes it holds
   unsigned long long* wave;   // device counters of the two-step kernel: err flag at [4], done1, done2 from [8]
   unsigned long long wave_epoch, wave_tickets;
+  unsigned long long strip_count[32];   // host mirror of the device's per-strip completion counters
   unsigned* order_dev;             // launch order table of the two-step kernel
   unsigned order_len;
   int order_key;                   // (D << 8) | nzf the tables were built for, -1: none
@@ -221,17 +222,32 @@ int launch_lb(nh_lattice* L) {
   return NH_OK;
 }
 // ---- two LB steps in one launch (nh_lb2.cuh) ----------------------------------------------------
-// Piece geometry for U cells per thread; false if this grid does not tile into pieces.
-struct PieceGrid { unsigned prows, ppr, rows_per_piece; int spr_shift; };
+// Geometry of one strip-plane for U cells per thread: YS lattice rows per strip (+ 2 halo rows in the
+// ring), cut into pieces of NT*U cells; false if this grid does not tile into pieces.
+struct PieceGrid { unsigned YS, nstrips, cps, ppr, rows_per_piece, pieces2; int spr_shift; };
 int lb2_threads(const nh_lattice* L) { return (L->options >> 31) & 1 ? 128 : 256; }
 bool piece_grid(const nh_lattice* L, int U, PieceGrid* g) {
   const unsigned nx = (unsigned)L->G.nx, ny = (unsigned)L->G.ny, seg = 32u * U, pc = (unsigned)lb2_threads(L) * U;
   const unsigned warps = (unsigned)lb2_threads(L) / 32;
   if (nx % seg) return false;
+  // strips of about 64 K cells per plane (what was measured to pay), or 2^c of them when forced
+  unsigned nstrips = 1;
+  const unsigned forced = (L->options >> 27) & 7u;
+  if (forced) nstrips = 1u << forced;
+  else while (nstrips < (unsigned)nh::WAVE_MAX_STRIPS && ny % (2 * nstrips) == 0 && (size_t)nx * (ny / (2 * nstrips)) >= 65536) nstrips *= 2;
+  if (nstrips > (unsigned)nh::WAVE_MAX_STRIPS || ny % nstrips) return false;
+  g->nstrips = nstrips;
+  g->YS = ny / nstrips;
   unsigned spr;
-  if (pc % nx == 0) { g->rows_per_piece = pc / nx; spr = nx / seg; g->prows = (ny + g->rows_per_piece - 1) / g->rows_per_piece; g->ppr = 1; }
-  else if (nx % pc == 0) { g->rows_per_piece = 1; spr = warps; g->prows = ny; g->ppr = nx / pc; }
-  else return false;
+  if (pc % nx == 0) {
+    g->rows_per_piece = pc / nx; spr = nx / seg; g->ppr = 1;
+    g->cps = (g->YS + 2 + g->rows_per_piece - 1) / g->rows_per_piece;
+    g->pieces2 = (g->YS + g->rows_per_piece - 1) / g->rows_per_piece;
+  } else if (nx % pc == 0) {
+    g->rows_per_piece = 1; spr = warps; g->ppr = nx / pc;
+    g->cps = (g->YS + 2) * g->ppr;
+    g->pieces2 = g->YS * g->ppr;
+  } else return false;
   g->spr_shift = 0;
   while ((1u << g->spr_shift) < spr) ++g->spr_shift;
   return (1u << g->spr_shift) == spr;
@@ -243,11 +259,14 @@ int lb2_cells_per_thread(const nh_lattice* L) {
   return 0;
 }
 // Ring and lead of the wavefront (planes).  Defaults from the B200 measurements in DESIGN.md.
-void lb2_lead(const nh_lattice* L, int* D, int* R) {
+void lb2_lead(const nh_lattice* L, const PieceGrid& g, int* D, int* R) {
   *D = (L->options >> 16) & 0xf; *R = (L->options >> 20) & 0x3f;
   if (*D == 0) *D = 4;
   if (*R == 0) *R = *D + 4;
-  if (*R > L->ring_cap) *R = L->ring_cap;
+  // the workspace holds ring_cap planes of (ny + 2) rows
+  const int cap = (int)((size_t)L->ring_cap * (L->G.ny + 2) / (g.YS + 2));
+  if (*R > cap) *R = cap;
+  if (*R > 63) *R = 63;
   if (*D > *R - 2) *D = *R - 2;
 }
 bool lb2_usable(const nh_lattice* L) {
@@ -255,14 +274,20 @@ bool lb2_usable(const nh_lattice* L) {
   if ((L->options & NH_OPT_LB_ONESTEP) || (L->options & NH_OPT_GRAPH) || L->ring_cap < 3) return false;
   const int U = lb2_cells_per_thread(L);
   if (U == 0) return false;
-  if (L->options & NH_OPT_LB_TWOSTEP) return true;
-  // automatic: only where it was measured to pay: FP32, a plane at least as
-  // large as the resident CTAs' work, and a ring that fits the L2 beside the streaming traffic
+  PieceGrid g;
+  piece_grid(L, U, &g);
   int D, R;
-  lb2_lead(L, &D, &R);
-  const double ring_mb = (double)R * 19.0 * L->G.plane * word_of(L->p.precision) / 1e6;
-  return word_of(L->p.precision) == 4 && L->G.plane >= 256u * 256u && ring_mb <= 48.0 && L->G.nz - 2 >= 4 * D;
+  lb2_lead(L, g, &D, &R);
+  if (R < 3 || D < 1) return false;
+  if (L->options & NH_OPT_LB_TWOSTEP) return true;
+  // automatic: only where it was measured to pay: FP32, a strip-plane at least as
+  // large as the resident CTAs' work, and a ring that fits the L2 beside the streaming traffic
+  const double ring_mb = (double)R * 19.0 * (g.YS + 2) * L->G.nx * word_of(L->p.precision) / 1e6;
+  return word_of(L->p.precision) == 4 && (size_t)g.YS * L->G.nx >= 65536 && ring_mb <= 48.0 && L->G.nz - 2 >= 4 * D;
 }
+
+// upper bound of the pieces of one strip-plane over all piece shapes (sizes the flag arrays)
+size_t lb2_max_pieces(int nx, int ny) { return (size_t)nx * (ny + 2) / 128 + ny + 3; }
 
 // Launch order of the wavefront: round j emits phase 2 of plane j-D-1, then phase 1 of plane j --
 // every unit after everything it waits for.
@@ -270,14 +295,13 @@ int lb2_order(nh_lattice* L, int D) {
   const int nzf = L->G.nz - 2;
   const int key = (D << 16) | nzf;
   if (L->order_key == key) return NH_OK;
-  const size_t pieces = (size_t)L->G.nx * L->G.ny / 128 + L->G.ny + 1;
   std::vector<unsigned> o;
   for (int j = 0; j < nzf + D + 1; ++j) {
     const int k2 = j - D - 1;
     if (k2 >= 0 && k2 < nzf) o.push_back((2u << 16) | (unsigned)k2);
     if (j < nzf) o.push_back((1u << 16) | (unsigned)j);
   }
-  L->order_dev = (unsigned*)(L->wave + 8 + (size_t)nzf * pieces);
+  L->order_dev = (unsigned*)(L->wave + 8 + nh::WAVE_MAX_STRIPS + (size_t)nzf * lb2_max_pieces(L->G.nx, L->G.ny));
   L->order_len = (unsigned)o.size();
   NH_CUDA(cudaMemcpyAsync(L->order_dev, o.data(), o.size() * sizeof(unsigned), cudaMemcpyHostToDevice, L->stream));
   NH_CUDA(cudaStreamSynchronize(L->stream));     // o goes out of scope
@@ -295,29 +319,38 @@ int launch_lb2_u(nh_lattice* L) {
   nh::Wave W;
   W.ticket = L->wave;
   W.err = (int*)(L->wave + 4);
-  W.prows = g.prows; W.ppr = g.ppr; W.rows_per_piece = g.rows_per_piece; W.spr_shift = g.spr_shift;
-  W.cps = g.prows * g.ppr;
-  W.flag1 = (unsigned*)(L->wave + 8);
+  W.strip_done = L->wave + 8;
+  W.YS = g.YS; W.nstrips = g.nstrips; W.cps = g.cps; W.ppr = g.ppr; W.rows_per_piece = g.rows_per_piece;
+  W.spr_shift = g.spr_shift;
+  W.rplane = (g.YS + 2) * (unsigned)L->G.nx;
+  W.flag1 = (unsigned*)(L->wave + 8 + nh::WAVE_MAX_STRIPS);
   W.flag2 = W.flag1 + (size_t)nzf * W.cps;
   W.nzf = nzf;
   int D, R;
-  lb2_lead(L, &D, &R);
+  lb2_lead(L, g, &D, &R);
   W.D = D; W.R = R;
   { const int rc = lb2_order(L, D); if (rc) return rc; }
   W.order = L->order_dev;
   W.reverse = next_sweep(L);
-  const unsigned long long units = (unsigned long long)L->order_len * W.cps;
+  W.units_per_strip = L->order_len * W.cps;
+  const unsigned long long units = (unsigned long long)W.units_per_strip * g.nstrips;
+  if (units >= 2147483648ull) return fail(NH_EINVAL, "two-step LB kernel: grid too large");
   if (L->options & NH_OPT_LB_BLOCKORDER) W.ticket = nullptr;
   W.ticket_base = L->wave_tickets;
   if (W.ticket) L->wave_tickets += units;   // one ticket per CTA
-  L->wave_epoch += 1;
-  W.epoch = (unsigned)L->wave_epoch;
+  W.epoch0 = (unsigned)L->wave_epoch + 1;   // strip s of this launch: epoch0 + s
+  L->wave_epoch += g.nstrips;
+  for (unsigned st = 0; st < g.nstrips; ++st) {
+    L->strip_count[st] += (unsigned long long)nzf * g.pieces2;
+    W.strip_target[st] = L->strip_count[st];
+  }
+  for (unsigned st = g.nstrips; st < (unsigned)nh::WAVE_MAX_STRIPS; ++st) W.strip_target[st] = 0;
   nh::DirTab<const T> A;
   nh::DirTab<T> Rg, B;
   for (int i = 0; i < nh::Q; ++i) {
     A.p[i] = (const T*)L->f[L->cur] + (size_t)i * L->G.N;
     B.p[i] = (T*)L->f[L->cur ^ 1] + (size_t)i * L->G.N;
-    Rg.p[i] = (T*)L->ring + (size_t)i * R * L->G.plane;
+    Rg.p[i] = (T*)L->ring + (size_t)i * R * W.rplane;
   }
   nh::lb_wave_kernel<T, SH, U, NT><<<(unsigned)units, NT, 0, L->stream>>>(A, Rg, B, (const T*)L->F, L->G, lb_const<T>(L), W);
   br.end();
@@ -714,7 +747,7 @@ size_t nh_workspace_bytes(const nh_params* p) {
   b += align_up(3 * N * sizeof(double));  // staging
   b += ALIGN;                      // flag
   if (three_constants(p)) b += align_up(9 * N * w) + 2 * align_up(3 * N * w);   // pi, df/dn, h
-  b += align_up((size_t)ring_planes(p) * 19 * p->nx * p->ny * w);   // plane ring of the two-step LB kernel
+  b += align_up((size_t)ring_planes(p) * 19 * p->nx * (p->ny + 2) * w);   // plane ring of the two-step LB kernel
   b += align_up(wave_words(p) * 8);                                 // its counters
   return b;
 }
@@ -755,9 +788,10 @@ int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_strea
   L->pi3 = L->dfdn3 = L->h3 = nullptr;
   if (three_constants(p)) { L->pi3 = take(9 * N * w); L->dfdn3 = take(3 * N * w); L->h3 = take(3 * N * w); }
   L->ring_cap = ring_planes(p);
-  L->ring = take((size_t)L->ring_cap * 19 * L->G.plane * w);
+  L->ring = take((size_t)L->ring_cap * 19 * L->G.nx * (L->G.ny + 2) * w);
   L->wave = (unsigned long long*)take(wave_words(p) * 8);
   L->wave_epoch = 0; L->wave_tickets = 0; L->order_key = -1;
+  for (int i = 0; i < 32; ++i) L->strip_count[i] = 0;
   e = cudaMemsetAsync(L->wave, 0, wave_words(p) * 8, L->stream);
   if (e != cudaSuccess) { delete L; return cuda_fail(e, "cudaMemsetAsync(wave)"); }
   int rc;

@@ -23,6 +23,13 @@
 //   is already running, so whatever a CTA waits for is running or done: no deadlock, no
 //   cooperative launch.  A wait longer than ~4 s sets an error flag instead of hanging the device.
 //
+// Strips.  The lattice is cut along y into strips of YS rows so that one strip-plane (YS x nx cells) is
+// what the resident CTAs can chew and R of them fit the L2 whatever the grid: the strips are done one
+// after the other, each with its own wavefront along z.  Phase 1 of a strip also computes the two
+// rows next to it (the ring plane has YS + 2 rows; ring row 0 / YS+1 are the lattice rows y0-1 /
+// y0+YS, periodic), so phase 2 needs nothing from another strip; the first R planes of a strip's
+// phase 1 wait until the previous strip has finished reading the ring.
+//
 // Each thread updates U cells 32 apart in x, so the address arithmetic is shared between them.
 // DRAM traffic per cell and PAIR of steps: 19 words read + 19 written (+ F^LC), against 2 x that
 // for two single launches; the ring traffic (19 written + 19 read) stays in the 126 MB L2.
@@ -33,22 +40,30 @@
 namespace nh {
 
 
+constexpr int WAVE_MAX_STRIPS = 32;
+
 struct Wave {
   unsigned long long* ticket;     // device counter, never reset
-  unsigned* flag1;                // [nzf][cps] launch number of the last finished phase-1 unit
+  unsigned* flag1;                // [nzf][cps] strip number (epoch) of the last finished phase-1 unit
   unsigned* flag2;                // the same for phase 2
+  unsigned long long* strip_done; // [nstrips] finished phase-2 units per strip, never reset
   int* err;                       // set to 1 if a wait timed out
   unsigned long long ticket_base; // value of *ticket when this launch starts
-  unsigned epoch;                 // this launch's number (> 0)
+  unsigned long long strip_target[WAVE_MAX_STRIPS];  // value of strip_done[s] when strip s of THIS launch is done
+  unsigned epoch0;                // flags of strip s of this launch carry epoch0 + s (> 0, grows across launches)
   int nzf;                        // fluid planes
-  unsigned cps;                   // pieces per plane = prows * ppr
-  unsigned prows, ppr;            // piece grid: piece rows, pieces per piece row
-  unsigned rows_per_piece;        // lattice rows of one piece (1 when a row holds several pieces)
-  int spr_shift;                  // log2(32*U-cell segments of one piece that lie in one lattice row)
+  unsigned YS;                    // lattice rows per strip (ny = nstrips * YS)
+  unsigned nstrips;
+  unsigned cps;                   // pieces per strip-plane of phase 1 (YS + 2 rows); phase 2 uses fewer
+  unsigned ppr;                   // pieces per row (1 when a piece holds whole rows)
+  unsigned rows_per_piece;        // rows of one piece (1 when a row holds several pieces)
+  unsigned units_per_strip;       // order_len * cps
+  unsigned rplane;                // cells of one ring plane = (YS + 2) * nx
+  int spr_shift;                  // log2(32*U-cell segments of one piece that lie in one row)
   int D;                          // lead of phase 1 over phase 2, in planes (>= 1)
   int R;                          // ring slots (planes), R >= D + 2
   int reverse;                    // sweep from the top plate down
-  const unsigned* order;          // [units per launch] (phase << 16) | logical plane, in launch order
+  const unsigned* order;          // [order_len] (phase << 16) | logical plane, in launch order
 };
 
 // p[i] = start of direction i inside a population array
@@ -63,30 +78,54 @@ __device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
   asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// 27 flags a unit depends on (3 planes x 3x3 pieces, periodic in the piece grid): lane l < 27
-// looks at one of them.  deps_look issues the acquire load and returns the flag (or "done" where
-// there is nothing to wait for); deps_test is the vote over the warp.
-__device__ __forceinline__ unsigned deps_look(const Wave& W, int phase, int k, unsigned prow, unsigned q,
-                                              unsigned lane) {
-  unsigned v = 0xffffffffu;
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+
+// The flags a unit depends on: 3 planes x up to 3 piece rows x 3 pieces along x (periodic in x; no
+// wrap along y: the ring has its own halo rows); lane l < 27 looks at one of them, lane 27 at the
+// previous strip.  prow counts piece rows inside the strip-plane of the unit's own phase:
+//   phase 2, piece row p: lattice rows p*rp .. = ring rows p*rp + 1 ..; it gathers ring rows
+//            p*rp .. (p+1)*rp + 1, i.e. phase-1 piece rows p .. ((p+1)*rp + 1)/rp
+//   phase 1, piece row p: ring rows p*rp .. (p+1)*rp - 1, read by the phase-2 piece rows
+//            p - (rp == 1 ? 2 : 1) .. p of the planes that used the slot before
+// Returns true when everything is in place.
+__device__ __forceinline__ bool deps_ready(const Wave& W, int phase, int k, unsigned strip, unsigned prow,
+                                           unsigned q, unsigned lane) {
+  bool ok = true;
+  const unsigned rp = W.rows_per_piece;
   if (lane < 27) {
     const int j = (phase == 2 ? k - 1 : k - W.R - 1) + (int)(lane / 9);
     if (j >= 0 && j < W.nzf) {
-      const unsigned r9 = lane % 9, dr = r9 / 3, dq = r9 % 3;      // 0, 1, 2 -> -1, 0, +1
-      unsigned pr = prow + dr, pq = q + dq;                        // periodic wrap without a division
-      pr = (pr == 0) ? W.prows - 1 : pr - 1;
-      if (pr == W.prows) pr = 0;
-      pq = (pq == 0) ? W.ppr - 1 : pq - 1;
-      if (pq == W.ppr) pq = 0;
-      v = ld_acquire_u32((phase == 2 ? W.flag1 : W.flag2) + (size_t)j * W.cps + pr * W.ppr + pq);
+      const unsigned r9 = lane % 9, dr = r9 / 3, dq = r9 % 3;
+      int p;
+      bool valid;
+      if (phase == 2) {
+        const unsigned last1 = (W.YS + 1) / rp;                    // last phase-1 piece row
+        unsigned hi = ((prow + 1) * rp + 1) / rp;
+        if (hi > last1) hi = last1;
+        p = (int)(prow + dr);
+        valid = (unsigned)p <= hi;
+      } else {
+        const int last2 = (int)((W.YS - 1) / rp);                  // last phase-2 piece row
+        p = (int)prow - (rp == 1 ? 2 : 1) + (int)dr;
+        valid = p >= 0 && p <= (int)prow && p <= last2;
+      }
+      if (valid) {
+        unsigned pq = q + dq;                                      // periodic along x, no division
+        pq = (pq == 0) ? W.ppr - 1 : pq - 1;
+        if (pq == W.ppr) pq = 0;
+        const unsigned* f = (phase == 2 ? W.flag1 : W.flag2) + (size_t)j * W.cps + (unsigned)p * W.ppr + pq;
+        ok = ld_acquire_u32(f) >= W.epoch0 + strip;
+      }
     }
+  } else if (lane == 27 && phase == 1 && strip > 0 && k < W.R) {
+    // the slot was last used by the previous strip: all of it must be done
+    ok = ld_acquire_u64(W.strip_done + (strip - 1)) >= W.strip_target[strip - 1];
   }
-  return v;
-}
-__device__ __forceinline__ bool deps_test(const Wave& W, unsigned v) { return __all_sync(0xffffffffu, v >= W.epoch); }
-__device__ __forceinline__ bool deps_ready(const Wave& W, int phase, int k, unsigned prow, unsigned q,
-                                           unsigned lane) {
-  return deps_test(W, deps_look(W, phase, k, prow, q, lane));
+  return __all_sync(0xffffffffu, ok);
 }
 
 // f_i(x, t) = f*_i(x - e_i, t-1) with half-way bounce-back for the U cells (xA + 32 j, y) of one
@@ -158,9 +197,9 @@ __device__ __forceinline__ void gather_cells(const Tab& S, unsigned zm, unsigned
 // NH_OPT_LB_BLOCKORDER the unit is blockIdx.x instead, which saves the atomic's round trip but relies
 // on CTAs being dispatched in blockIdx order (the hardware does, CUDA does not promise it; the
 // bounded waits turn a violation into an error flag, not a hang).  No loop-carried state; each warp
-// checks the flags itself (27 lanes, one acquire load).  A phase-1 unit gathers first and checks
+// checks the flags itself (28 lanes, one acquire load).  A phase-1 unit gathers first and checks
 // its flags (the old readers of its ring slot) only before it stores; a phase-2 unit checks before
-// it gathers.  One barrier at the end, then thread 0 publishes the unit with a store-release.
+// it gathers.  One barrier at the end, then thread 0 publishes the unit (fence, flag, counter).
 template <typename T, bool SHIFTED, int U, int NT>
 __global__ void __launch_bounds__(NT, (sizeof(T) == 4 ? 4 : (U == 2 ? 1 : 2)) * (256 / NT))
 lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restrict__ Flc,
@@ -169,55 +208,67 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
   // which unit: decoded once (by thread 0 from its ticket, or by everyone from blockIdx, which the
   // compiler keeps on the uniform datapath)
   int phase, k;
-  unsigned prow, q;
+  unsigned strip, prow, q;
+  auto decode = [&](unsigned tk, int& ph, int& kk, unsigned& st, unsigned& pr, unsigned& qq) {
+    st = tk / W.units_per_strip;
+    const unsigned rem = tk - st * W.units_per_strip;
+    const unsigned unit = rem / W.cps, piece = rem - unit * W.cps;
+    const unsigned code = W.order[unit];
+    ph = (int)(code >> 16); kk = (int)(code & 0xffffu);
+    pr = piece / W.ppr; qq = piece - pr * W.ppr;
+  };
   if (W.ticket) {                       // safe order: a ticket drawn when the CTA starts to run
-    __shared__ int s_unit[4];
+    __shared__ unsigned s_unit[5];
     if (threadIdx.x == 0) {
-      const unsigned tk = (unsigned)(atomicAdd(W.ticket, 1ull) - W.ticket_base);
-      const unsigned unit = tk / W.cps, piece = tk - unit * W.cps;
-      const unsigned code = W.order[unit];
-      s_unit[0] = (int)(code >> 16); s_unit[1] = (int)(code & 0xffffu); s_unit[2] = (int)(piece / W.ppr); s_unit[3] = (int)(piece % W.ppr);
+      int ph, kk;
+      unsigned st, pr, qq;
+      decode((unsigned)(atomicAdd(W.ticket, 1ull) - W.ticket_base), ph, kk, st, pr, qq);
+      s_unit[0] = (unsigned)ph; s_unit[1] = (unsigned)kk; s_unit[2] = st; s_unit[3] = pr; s_unit[4] = qq;
     }
     __syncthreads();
-    phase = s_unit[0]; k = s_unit[1]; prow = (unsigned)s_unit[2]; q = (unsigned)s_unit[3];
+    phase = (int)s_unit[0]; k = (int)s_unit[1]; strip = s_unit[2]; prow = s_unit[3]; q = s_unit[4];
   } else {
-    const unsigned unit = blockIdx.x / W.cps, piece = blockIdx.x - unit * W.cps;
-    const unsigned code = W.order[unit];
-    phase = (int)(code >> 16); k = (int)(code & 0xffffu);
-    prow = piece / W.ppr; q = piece - prow * W.ppr;
+    decode(blockIdx.x, phase, k, strip, prow, q);
   }
+  const unsigned row_local = prow * W.rows_per_piece + (warp >> W.spr_shift);   // row inside the piece grid
+  // phase 2 has two rows fewer than phase 1: its surplus pieces are empty
+  if (phase == 2 && prow * W.rows_per_piece >= W.YS) return;
   auto wait_flags = [&]() {
     const long long t0 = clock64();
     unsigned ns = 32;
-    while (!deps_ready(W, phase, k, prow, q, lane)) {
+    while (!deps_ready(W, phase, k, strip, prow, q, lane)) {
       __nanosleep(ns);
       if (ns < 512) ns *= 2;
       if (clock64() - t0 > 8000000000ll) { if (lane == 0) atomicExch(W.err, 1); break; }
     }
   };
-  const unsigned seg_row = warp >> W.spr_shift;
+  const unsigned nx = (unsigned)G.nx, ny = (unsigned)G.ny;
   const unsigned seg_x = (warp & ((1u << W.spr_shift) - 1u)) * (32u * U);
   const int z = (W.reverse ? W.nzf - 1 - k : k) + 1;
-  const unsigned y = prow * W.rows_per_piece + seg_row;
   const unsigned xA = q * (unsigned)(NT * U) + seg_x + lane;
-  const bool active = y < (unsigned)G.ny;
-  const unsigned nx = (unsigned)G.nx;
-  const unsigned r0 = y * nx;
+  const unsigned y0 = strip * W.YS;
+  // ring row and lattice row of this thread's cells
+  const unsigned ry = (phase == 1) ? row_local : row_local + 1;
+  const bool active = (phase == 1) ? (row_local < W.YS + 2) : (row_local < W.YS);
+  unsigned y = y0 + ry;                               // = lattice row + 1
+  y = (y == 0) ? ny - 1 : y - 1;
+  if (y >= ny) y -= ny;
   const unsigned slot = (unsigned)((z - 1) % W.R);
-  const unsigned cell = (unsigned)z * G.plane + r0 + xA;
+  const unsigned cell = (unsigned)z * G.plane + y * nx + xA;
+  const unsigned rcell = slot * W.rplane + ry * nx + xA;
   if (phase == 2) wait_flags();
   Pop<T> P[U];
   T Fx[U], Fy[U], Fz[U];
   if (active) {
-    const unsigned rm = (y == 0 ? (unsigned)G.ny - 1 : y - 1) * nx;
-    const unsigned rp = (y == (unsigned)G.ny - 1 ? 0u : y + 1) * nx;
     const bool lo = (z == 1), hi = (z == G.nz - 2);
     if (phase == 1) {
       const unsigned z0 = (unsigned)z * G.plane;
-      gather_cells<T, LD_CS, U>(A, z0 - G.plane, z0, z0 + G.plane, r0, rm, rp, xA, nx, lo, hi, P);
+      const unsigned rm = (y == 0 ? ny - 1 : y - 1) * nx, rp = (y == ny - 1 ? 0u : y + 1) * nx;
+      gather_cells<T, LD_CS, U>(A, z0 - G.plane, z0, z0 + G.plane, y * nx, rm, rp, xA, nx, lo, hi, P);
     } else {
       const unsigned sm = (slot == 0 ? (unsigned)W.R - 1 : slot - 1), sp = (slot == (unsigned)W.R - 1 ? 0u : slot + 1);
-      gather_cells<T, LD_CG, U>(ring, sm * G.plane, slot * G.plane, sp * G.plane, r0, rm, rp, xA, nx, lo, hi, P);
+      gather_cells<T, LD_CG, U>(ring, sm * W.rplane, slot * W.rplane, sp * W.rplane, ry * nx, (ry - 1) * nx,
+                                (ry + 1) * nx, xA, nx, lo, hi, P);
     }
 #pragma unroll
     for (int j = 0; j < U; ++j) {
@@ -228,19 +279,18 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
       }
     }
   }
-  unsigned look = 0xffffffffu;
-  if (phase == 1) look = deps_look(W, phase, k, prow, q, lane);
+  bool ready = true;
+  if (phase == 1) ready = deps_ready(W, phase, k, strip, prow, q, lane);   // a look while the gathers fly
   if (active) {
 #pragma unroll
     for (int j = 0; j < U; ++j) collide<T, SHIFTED>(P[j], Fx[j], Fy[j], Fz[j], C);
   }
-  if (phase == 1 && !deps_test(W, look)) wait_flags();
+  if (phase == 1 && !ready) wait_flags();
   if (active) {
     if (phase == 1) {
-      const unsigned o = slot * G.plane + r0 + xA;
 #pragma unroll
       for (int i = 0; i < Q; ++i) {
-        T* d = ring.p[i] + o;
+        T* d = ring.p[i] + rcell;
 #pragma unroll
         for (int j = 0; j < U; ++j) d[32 * j] = P[j].f[i];
       }
@@ -254,8 +304,13 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
     }
   }
   __syncthreads();
-  if (threadIdx.x == 0)
-    st_release_u32((phase == 1 ? W.flag1 : W.flag2) + (size_t)k * W.cps + prow * W.ppr + q, W.epoch);
+  if (threadIdx.x == 0) {
+    // publish: everything this CTA read and wrote is ordered before the flag (and the strip counter)
+    __threadfence();
+    unsigned* f = (phase == 1 ? W.flag1 : W.flag2) + (size_t)k * W.cps + prow * W.ppr + q;
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(f), "r"(W.epoch0 + strip) : "memory");
+    if (phase == 2) asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(W.strip_done + strip), "l"(1ull) : "memory");
+  }
 }
 
 }  // namespace nh

@@ -37,10 +37,10 @@ def test_workspace_bytes_and_validation(lib):
     b32 = nh.workspace_bytes(p)
     # populations A, B; n, n', n^P, a, u, F; FP64 staging; the two-step kernel's plane ring
     # (min(nz-2, 12) planes of 19 populations) and its flags (include/nh.h)
-    ring = min(8 - 2, 12) * 19 * 16 * 16
+    ring = min(8 - 2, 12) * 19 * 16 * (16 + 2)          # ring planes have two halo rows
     fields32 = (2 * 19 + 6 * 3) * N * 4 + 3 * N * 8 + ring * 4
     assert b32 >= fields32
-    assert b32 <= fields32 + 12 * 256 + 8 * (8 + 6 * (16 * 16 // 128 + 16 + 1))
+    assert b32 <= fields32 + 12 * 256 + 8 * (8 + 32 + 6 * (16 * 18 // 128 + 16 + 3) + 6 + 8)
     p64 = nh.make_params(16, 16, 8, 0.8, precision=nh.FP64_SHIFTED)
     assert nh.workspace_bytes(p64) >= (2 * 19 + 6 * 3) * N * 8 + 3 * N * 8 + ring * 8
     for bad in (dict(tau=0.5), dict(nz=2), dict(gamma1=0.0), dict(K=-1.0), dict(fd_ratio=-1),

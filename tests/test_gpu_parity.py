@@ -229,7 +229,8 @@ def test_options_do_not_change_results():
 
 
 @pytest.mark.parametrize("shape,r", [((64, 64, 32), 10), ((128, 5, 20), 7), ((32, 7, 9), 3), ((512, 4, 6), 2),
-                                     ((1024, 3, 5), 2), ((64, 3, 3), 2), ((256, 9, 8), 4), ((16, 16, 8), 1)])
+                                     ((1024, 3, 5), 2), ((64, 3, 3), 2), ((256, 9, 8), 4), ((16, 16, 8), 1),
+                                     ((128, 24, 12), 3), ((512, 16, 9), 4), ((64, 40, 7), 2)])
 def test_two_step_kernel_is_bit_identical(shape, r):
     """The two-steps-per-sweep LB kernel (L2-resident plane ring, wavefront along z) does the same
     arithmetic per cell as the one-step kernel, so every field must agree bit for bit, whatever
@@ -254,7 +255,8 @@ def test_two_step_kernel_is_bit_identical(shape, r):
     for precision in (0, 1):
         ref = run(precision, m.OPT_LB_ONESTEP, [43])
         for opt in (T, T | m.OPT_NO_SERPENTINE, T | (1 << 30), T | (1 << 31), T | (1 << 16) | (3 << 20),
-                    T | (3 << 16) | (12 << 20) | m.OPT_LB_BLOCKORDER, T | m.OPT_LB_BLOCKORDER | (1 << 30)):
+                    T | (3 << 16) | (12 << 20) | m.OPT_LB_BLOCKORDER, T | m.OPT_LB_BLOCKORDER | (1 << 30),
+                    T | (1 << 27), T | (2 << 27) | (2 << 16) | (5 << 20), T | (3 << 27) | m.OPT_LB_BLOCKORDER):   # 2, 4, 8 strips
             f = run(precision, opt, [1, 7, 20, 15])
             for k in ref:
                 assert np.array_equal(ref[k], f[k]), (shape, precision, hex(opt), k)
