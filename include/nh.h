@@ -127,13 +127,16 @@ long nh_launch_count(const nh_lattice* L);
  *   bit5 NH_OPT_FD_NOVEC      stage the FD tiles element by element even where 16-byte copies fit
  *   bit6 NH_OPT_LB_TWOSTEP    two LB steps per launch through an L2-resident plane ring wherever no
  *                             director update falls between them and the grid tiles into pieces
- *                             (nx a multiple of 64 that divides, or is a multiple of, 512);
+ *                             (nx a multiple of 64 that divides, or is a multiple of, 512; else one step
+ *                             per launch);
  *                             bit-identical results.  Without bit6 and bit7 the library decides
  *                             (FP32, planes >= 256x256, ring <= 48 MB: DESIGN.md section 7).
  *   bit7 NH_OPT_LB_ONESTEP    never use the two-step kernel
  *   bits 8-15                 planes per CTA of the tiled FD kernels (0 = chosen by the library)
  *   bits 16-19, 20-25         two-step kernel: lead D of phase 1 in planes, ring planes R (0 = default)
  *   bit26 NH_OPT_LB_BLOCKORDER two-step kernel: units in blockIdx order instead of by atomic ticket
+ *   bits 27-29                two-step kernel: log2 of the number of y-strips (0 = chosen by the library:
+ *                             strips of about 64 K cells per plane; ny must be divisible by it)
  *   bits 30, 31               two-step kernel: one cell per thread; 128-thread CTAs (tuning)
  * Setting options resets the timing accumulators. */
 #define NH_OPT_GRAPH          1

@@ -15,10 +15,11 @@
 //   one plane of one phase, done by one CTA.  Units are ordered -- phase 1 of planes 0..D, then
 //   phase 2 of plane k and phase 1 of plane k+D+1 alternating, piece by piece inside a plane -- and
 //   a CTA takes the next unit from an atomic ticket counter when it starts to run.
-//   Dependencies are per-piece flags in global memory holding the launch number:
-//     phase 2 of (k, piece)  needs phase 1 of planes k-1, k, k+1 at the 3x3 neighbouring pieces
-//     phase 1 of (k, piece)  needs phase 2 of planes k-R-1 .. k-R+1 at the same pieces (the readers
-//                            of the ring slot it overwrites)
+//   Dependencies are per-piece flags in global memory holding a number that grows with every
+//   launch and strip:
+//     phase 2 of (k, piece)  needs phase 1 of planes k-1, k, k+1 at the neighbouring pieces
+//     phase 1 of (k, piece)  needs phase 2 of planes k-R-1 .. k-R+1 at the pieces that read the
+//                            ring slot it overwrites
 //   Every unit depends only on units EARLIER in ticket order, and a ticket is drawn by a CTA that
 //   is already running, so whatever a CTA waits for is running or done: no deadlock, no
 //   cooperative launch.  A wait longer than ~4 s sets an error flag instead of hanging the device.
@@ -73,9 +74,6 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
   unsigned v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
-}
-__device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
-  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
@@ -208,7 +206,7 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
   // which unit: decoded once (by thread 0 from its ticket, or by everyone from blockIdx, which the
   // compiler keeps on the uniform datapath)
   int phase, k;
-  unsigned strip, prow, q;
+  unsigned strip, prow, q, slot;
   auto decode = [&](unsigned tk, int& ph, int& kk, unsigned& st, unsigned& pr, unsigned& qq) {
     st = tk / W.units_per_strip;
     const unsigned rem = tk - st * W.units_per_strip;
@@ -218,17 +216,20 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
     pr = piece / W.ppr; qq = piece - pr * W.ppr;
   };
   if (W.ticket) {                       // safe order: a ticket drawn when the CTA starts to run
-    __shared__ unsigned s_unit[5];
+    __shared__ unsigned s_unit[6];
     if (threadIdx.x == 0) {
       int ph, kk;
       unsigned st, pr, qq;
       decode((unsigned)(atomicAdd(W.ticket, 1ull) - W.ticket_base), ph, kk, st, pr, qq);
       s_unit[0] = (unsigned)ph; s_unit[1] = (unsigned)kk; s_unit[2] = st; s_unit[3] = pr; s_unit[4] = qq;
+      s_unit[5] = (unsigned)((W.reverse ? W.nzf - 1 - kk : kk) % W.R);     // ring slot of the plane
     }
     __syncthreads();
     phase = (int)s_unit[0]; k = (int)s_unit[1]; strip = s_unit[2]; prow = s_unit[3]; q = s_unit[4];
+    slot = s_unit[5];
   } else {
     decode(blockIdx.x, phase, k, strip, prow, q);
+    slot = (unsigned)((W.reverse ? W.nzf - 1 - k : k) % W.R);
   }
   const unsigned row_local = prow * W.rows_per_piece + (warp >> W.spr_shift);   // row inside the piece grid
   // phase 2 has two rows fewer than phase 1: its surplus pieces are empty
@@ -253,7 +254,6 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
   unsigned y = y0 + ry;                               // = lattice row + 1
   y = (y == 0) ? ny - 1 : y - 1;
   if (y >= ny) y -= ny;
-  const unsigned slot = (unsigned)((z - 1) % W.R);
   const unsigned cell = (unsigned)z * G.plane + y * nx + xA;
   const unsigned rcell = slot * W.rplane + ry * nx + xA;
   if (phase == 2) wait_flags();
