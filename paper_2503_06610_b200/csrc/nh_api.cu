@@ -442,11 +442,28 @@ int launch_force(nh_lattice* L) {
   const T* u = (const T*)L->u;
   if (three_constants(&L->p)) {
     br.end();
-    { const int rc = launch_h3<T>(L, n, KC_FORCE); if (rc) return rc; }
+    const bool tiled3 = !(L->options & NH_OPT_FD_DIRECT) && tiles_fit(L);
+    // h (through pi) is needed by the viscous stress, and by the one-thread-per-cell form always
+    if (C.visc || !tiled3) { const int rc = launch_h3<T>(L, n, KC_FORCE); if (rc) return rc; }
     Bracket b3(L, KC_FORCE);
     if (b3.rc) return b3.rc;
-    nh::force3_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(n, u, (const T*)L->pi3, (const T*)L->h3,
-                                                                          (T*)L->F, L->G, C);
+    if (tiled3) {
+      const TileGrid g = tile_grid(L);
+      const nh::Frank3<T> K3 = frank3_const<T>(L);
+      const T* hb = (const T*)L->h3;
+      if (C.visc) {
+        const size_t sm = nh::force_smem_bytes<T, true>();
+        if (tiles_vec(L)) nh::force_tile_kernel<T, true, true, true><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(n, u, (T*)L->F, L->G, C, g.zchunk, K3, hb);
+        else nh::force_tile_kernel<T, false, true, true><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(n, u, (T*)L->F, L->G, C, g.zchunk, K3, hb);
+      } else {
+        const size_t sm = nh::force_smem_bytes<T, false>();
+        if (tiles_vec(L)) nh::force_tile_kernel<T, true, false, true><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(n, u, (T*)L->F, L->G, C, g.zchunk, K3, hb);
+        else nh::force_tile_kernel<T, false, false, true><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(n, u, (T*)L->F, L->G, C, g.zchunk, K3, hb);
+      }
+    } else {
+      nh::force3_kernel<T><<<blocks_for(L->G.nfluid), BLOCK, 0, L->stream>>>(n, u, (const T*)L->pi3, (const T*)L->h3,
+                                                                            (T*)L->F, L->G, C);
+    }
     b3.end();
     return NH_OK;
   }
@@ -556,6 +573,10 @@ int enable_tile_smem() {
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false, false>, attr, fb));
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, true, true>, attr, fvb));
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false, true>, attr, fvb));
+  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, true, false, true>, attr, fb));
+  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false, false, true>, attr, fb));
+  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, true, true, true>, attr, fvb));
+  NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false, true, true>, attr, fvb));
   return NH_OK;
 }
 

@@ -22,6 +22,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include "nh_fd.cuh"
+#include "nh_frank3.cuh"
 
 namespace nh {
 
@@ -290,11 +291,35 @@ __device__ __forceinline__ void stress_all(const FdConst<T>& C, V3<T> n, V3<T> d
   sz = {C.Kq0 * cx.z - C.K * gxz, C.Kq0 * cy.z - C.K * gyz, C.Kq0 * cz.z - C.K * gzz};
 }
 
+// three-constant energy (row f2): sigma^e_{a b} = -d_a n_c pi_{b c} with the LOCAL pi of nh_frank3.cuh;
+// the viscous part takes h from the buffer that h3_kernel has filled (h needs pi at the neighbours)
+template <typename T>
+__device__ __forceinline__ void stress3_staged(const FdConst<T>& C, const Frank3<T>& K3, bool visc,
+                                               const T* nzm, const T* nc, const T* nzp,
+                                               const T* uzm, const T* uc, const T* uzp, int o,
+                                               const T* __restrict__ hbuf, unsigned cell, unsigned N, bool cell_ok,
+                                               V3<T>& sx, V3<T>& sy, V3<T>& sz) {
+  V3<T> n, dxn, dyn, dzn, px, py, pz, dfdn;
+  grad_staged(nzm, nc, nzp, o, n, dxn, dyn, dzn);
+  frank3_local(K3, n, dxn, dyn, dzn, px, py, pz, dfdn);
+  sx = {-dot(dxn, px), -dot(dyn, px), -dot(dzn, px)};
+  sy = {-dot(dxn, py), -dot(dyn, py), -dot(dzn, py)};
+  sz = {-dot(dxn, pz), -dot(dyn, pz), -dot(dzn, pz)};
+  if (visc) {
+    V3<T> u0, dxu, dyu, dzu;
+    grad_staged(uzm, uc, uzp, o, u0, dxu, dyu, dzu);
+    V3<T> h = {T(0), T(0), T(0)};
+    if (cell_ok) h = {hbuf[cell], hbuf[cell + N], hbuf[cell + 2 * N]};
+    viscous_add_h(C, n, C.inv_gamma1 * h, dxu, dyu, dzu, sx, sy, sz);
+  }
+}
+
 // VISC: the Leslie viscous stress is added (Eq. 12 in full, row f1): u is staged like n.
-template <typename T, bool VEC, bool VISC>
+// FR3: three-constant Frank energy (K3, hbuf).
+template <typename T, bool VEC, bool VISC, bool FR3 = false>
 __global__ void __launch_bounds__(TILE_THREADS)
 force_tile_kernel(const T* __restrict__ n, const T* __restrict__ u, T* __restrict__ Fout, Geom G,
-                  FdConst<T> C, int zchunk) {
+                  FdConst<T> C, int zchunk, Frank3<T> K3 = Frank3<T>(), const T* __restrict__ hbuf = nullptr) {
   using S = PlaneShape<2>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* sn = reinterpret_cast<T*>(smem_raw);                 // [FORCE_SLOTS][S::ELEMS]
@@ -315,6 +340,10 @@ force_tile_kernel(const T* __restrict__ n, const T* __restrict__ u, T* __restric
   st.init(G, x0, y0);
   // face-halo duty of threads 0..79: which staged cell, which column (0: sigma_.x, 1: sigma_.y)
   int hn = -1, hs = 0, hcol = 0;
+  unsigned hcell = 0;                                     // in-plane index of the halo cell (FR3 + VISC: h buffer)
+  // in-plane index of the own cell, wrapped: threads hanging over the edge of the lattice still
+  // compute sigma for their periodic image, which active neighbours read
+  const unsigned ownw = (unsigned)(y % G.ny) * (unsigned)G.nx + (unsigned)(x % G.nx);
   {
     const int t = threadIdx.x;
     int hx = 0, hy = 0;                                    // tile-relative, -1 .. TX / TY
@@ -323,6 +352,9 @@ force_tile_kernel(const T* __restrict__ n, const T* __restrict__ u, T* __restric
     if (t < 2 * TX + 2 * TY) {
       hn = (hy + 2) * S::RS + S::CO + hx;
       hs = (hy + 1) * SigShape::PX + (hx + 1) + 3 * hcol * SigShape::CELLS;
+      int gx = (x0 + hx) % G.nx; if (gx < 0) gx += G.nx;
+      int gy = (y0 + hy) % G.ny; if (gy < 0) gy += G.ny;
+      hcell = (unsigned)gy * (unsigned)G.nx + (unsigned)gx;
     }
   }
   const int pfirst = z0 - 1, plast = z1 + 1;
@@ -368,7 +400,9 @@ force_tile_kernel(const T* __restrict__ n, const T* __restrict__ u, T* __restric
       const T* uzm = su + ((p - 1) & 3) * S::ELEMS;
       const T* uc = su + (p & 3) * S::ELEMS;
       const T* uzp = su + ((p + 1) & 3) * S::ELEMS;
-      if (VISC) {
+      if (FR3) {
+        stress3_staged(C, K3, VISC, pzm, pc, pzp, uzm, uc, uzp, on, hbuf, ownw + (unsigned)p * G.plane, N, true, sx, sy, szC);
+      } else if (VISC) {
         stress_visc_staged(C, pzm, pc, pzp, uzm, uc, uzp, on, sx, sy, szC);
       } else {
         grad_staged(pzm, pc, pzp, on, nn, dxn, dyn, dzn);
@@ -378,7 +412,12 @@ force_tile_kernel(const T* __restrict__ n, const T* __restrict__ u, T* __restric
       sig[3 * SigShape::CELLS + os] = sy.x; sig[4 * SigShape::CELLS + os] = sy.y; sig[5 * SigShape::CELLS + os] = sy.z;
       if (hn >= 0) {
         V3<T> sh;
-        if (VISC) {
+        if (FR3) {
+          // the halo cell's index: same plane, tile-relative (hx, hy) wrapped periodically
+          V3<T> hx, hy, hz;
+          stress3_staged(C, K3, VISC, pzm, pc, pzp, uzm, uc, uzp, hn, hbuf, hcell + (unsigned)p * G.plane, N, true, hx, hy, hz);
+          sh = hcol == 0 ? hx : hy;
+        } else if (VISC) {
           V3<T> hx, hy, hz;
           stress_visc_staged(C, pzm, pc, pzp, uzm, uc, uzp, hn, hx, hy, hz);
           sh = hcol == 0 ? hx : hy;
