@@ -502,6 +502,36 @@ int launch_director(nh_lattice* L, int r) {
   const nh::FdConst<T> C = fd_const<T>(L, r);
   const bool tiled = !(L->options & NH_OPT_FD_DIRECT) && tiles_fit(L);
   const TileGrid g = tile_grid(L);
+  if (three_constants(&L->p) && tiled) {
+    const nh::Frank3<T> K3 = frank3_const<T>(L);
+    const size_t sm = nh::force_smem_bytes<T, true>();
+    {
+      Bracket br(L, KC_PRED);
+      if (br.rc) return br.rc;
+      if (tiles_vec(L))
+        nh::director3_tile_kernel<T, 0, true><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(
+            (const T*)L->n[L->ncur], (const T*)L->u, nullptr, (T*)L->nP, (T*)L->a, L->G, C, K3, with_flow, g.zchunk);
+      else
+        nh::director3_tile_kernel<T, 0, false><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(
+            (const T*)L->n[L->ncur], (const T*)L->u, nullptr, (T*)L->nP, (T*)L->a, L->G, C, K3, with_flow, g.zchunk);
+      br.end();
+    }
+    int rc = mirror_plates<T>(L, L->nP);
+    if (rc) return rc;
+    {
+      Bracket br(L, KC_CORR);
+      if (br.rc) return br.rc;
+      if (tiles_vec(L))
+        nh::director3_tile_kernel<T, 1, true><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(
+            (const T*)L->nP, (const T*)L->u, (const T*)L->a, (T*)L->n[L->ncur ^ 1], nullptr, L->G, C, K3, with_flow, g.zchunk);
+      else
+        nh::director3_tile_kernel<T, 1, false><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(
+            (const T*)L->nP, (const T*)L->u, (const T*)L->a, (T*)L->n[L->ncur ^ 1], nullptr, L->G, C, K3, with_flow, g.zchunk);
+      br.end();
+    }
+    L->ncur ^= 1;
+    return mirror_plates<T>(L, L->n[L->ncur]);
+  }
   if (three_constants(&L->p)) {
     int rc = launch_h3<T>(L, L->n[L->ncur], KC_PRED);
     if (rc) return rc;
@@ -573,6 +603,10 @@ int enable_tile_smem() {
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false, false>, attr, fb));
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, true, true>, attr, fvb));
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false, true>, attr, fvb));
+  NH_CUDA(cudaFuncSetAttribute(nh::director3_tile_kernel<T, 0, true>, attr, fvb));
+  NH_CUDA(cudaFuncSetAttribute(nh::director3_tile_kernel<T, 1, true>, attr, fvb));
+  NH_CUDA(cudaFuncSetAttribute(nh::director3_tile_kernel<T, 0, false>, attr, fvb));
+  NH_CUDA(cudaFuncSetAttribute(nh::director3_tile_kernel<T, 1, false>, attr, fvb));
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, true, false, true>, attr, fb));
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false, false, true>, attr, fb));
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, true, true, true>, attr, fvb));

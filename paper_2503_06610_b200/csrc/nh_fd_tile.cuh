@@ -446,4 +446,141 @@ force_tile_kernel(const T* __restrict__ n, const T* __restrict__ u, T* __restric
   cp_async_wait_all();
 }
 
+// ---- predictor / corrector with the three-constant energy (row f2) --------------------------------
+// h_m = -df/dn_m + d_b pi_{b m} needs pi at the six neighbours, so the march is the force kernel's:
+// at plane p every thread evaluates pi (rows pi_x., pi_y. to a double-buffered shared plane, pi_z. in
+// registers) and df/dn at its own cell, the first 80 threads also the row the tile's face halo needs;
+// one plane later h of plane p-1 is complete and the director's rate follows (flow terms and
+// projection shared with the one-constant path).  The own cell's column of m and u is carried in
+// registers (plane p-2 is being overwritten in the ring by then).
+//   STAGE 0: out_m = n^P = unit(m + dt k1), a_out = m + dt/2 k1;  STAGE 1: out_m = unit(a_in + dt/2 k2)
+template <typename T, int STAGE, bool VEC>
+__global__ void __launch_bounds__(TILE_THREADS)
+director3_tile_kernel(const T* __restrict__ m, const T* __restrict__ u, const T* __restrict__ a_in,
+                      T* __restrict__ out_m, T* __restrict__ a_out, Geom G, FdConst<T> C, Frank3<T> K3,
+                      int with_flow, int zchunk) {
+  using S = PlaneShape<2>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* sn = reinterpret_cast<T*>(smem_raw);                 // [FORCE_SLOTS][S::ELEMS]  m
+  T* ssig = sn + FORCE_SLOTS * S::ELEMS;                  // [2][SigShape::ELEMS]     pi_x., pi_y.
+  T* su = ssig + 2 * SigShape::ELEMS;                     // [FORCE_SLOTS][S::ELEMS]  u
+  const unsigned su_addr = smem_u32(su);
+  const int tx = threadIdx.x % TX, ty = threadIdx.x / TX;
+  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+  const int z0 = 1 + blockIdx.z * zchunk;
+  const int z1 = min(z0 + zchunk - 1, G.nz - 2);
+  const int x = x0 + tx, y = y0 + ty;
+  const bool active = (x < G.nx) && (y < G.ny);
+  const bool flow = with_flow != 0;
+  const int on = (ty + 2) * S::RS + S::CO + tx;
+  const int os = (ty + 1) * SigShape::PX + (tx + 1);
+  constexpr unsigned SLOT_BYTES = S::ELEMS * sizeof(T);
+  const unsigned sn_addr = smem_u32(sn);
+  Stager<T, 2, VEC> st;
+  st.init(G, x0, y0);
+  int hn = -1, hs = 0, hcol = 0;
+  {
+    const int t = threadIdx.x;
+    int hx = 0, hy = 0;
+    if (t < 2 * TX) { hx = t % TX; hy = (t < TX) ? -1 : TY; hcol = 1; }
+    else if (t < 2 * TX + 2 * TY) { const int q = t - 2 * TX; hy = q % TY; hx = (q < TY) ? -1 : TX; hcol = 0; }
+    if (t < 2 * TX + 2 * TY) {
+      hn = (hy + 2) * S::RS + S::CO + hx;
+      hs = (hy + 1) * SigShape::PX + (hx + 1) + 3 * hcol * SigShape::CELLS;
+    }
+  }
+  const int pfirst = z0 - 1, plast = z1 + 1;
+  const int zlo = max(pfirst - 1, 0), zhi = min(plast + 1, G.nz - 1);
+  int zf = zlo;
+  const T* src = m + (size_t)zlo * G.plane;
+  const T* usrc = u + (size_t)zlo * G.plane;
+  for (; zf <= zlo + 2; ++zf) {
+    st.fetch(src, sn_addr + (zf & 3) * SLOT_BYTES);
+    if (flow) st.fetch(usrc, su_addr + (zf & 3) * SLOT_BYTES);
+    src += G.plane; usrc += G.plane;
+  }
+  cp_async_commit();
+  const V3<T> zero = {T(0), T(0), T(0)};
+  V3<T> pzA = zero, pzB = zero;                           // pi_z. at planes p-2, p-1
+  V3<T> dfB = zero;                                       // df/dn at plane p-1
+  V3<T> mA = zero, mB = zero, uA = zero, uB = zero;       // own cell of m, u at planes p-2, p-1
+  unsigned c = (unsigned)(z0 - 1) * G.plane + (unsigned)y * (unsigned)G.nx + (unsigned)x;   // cell (x, y, p)
+  const unsigned N = (unsigned)G.N;
+  const T hdt = T(0.5) * C.dt;
+
+  for (int p = pfirst; p <= plast; ++p) {
+    cp_async_wait_all();
+    __syncthreads();
+    if (zf <= zhi && zf <= p + 2) {
+      st.fetch(src, sn_addr + (zf & 3) * SLOT_BYTES);
+      if (flow) st.fetch(usrc, su_addr + (zf & 3) * SLOT_BYTES);
+      src += G.plane; usrc += G.plane; ++zf;
+    }
+    cp_async_commit();
+    T* sig = ssig + (p & 1) * SigShape::ELEMS;
+    const T* pc = sn + (p & 3) * S::ELEMS;
+    const T* pzm = sn + ((p - 1) & 3) * S::ELEMS;
+    const T* pzp = sn + ((p + 1) & 3) * S::ELEMS;
+    const bool plate = (p == 0 || p == G.nz - 1);
+    // pi and df/dn of plane p at the own cell (zero gradient inside the plates)
+    V3<T> mC, dxm = zero, dym = zero, dzm = zero, px, py, pzC, dfC;
+    if (plate) mC = lds3<T, 2>(pc, on);
+    else grad_staged(pzm, pc, pzp, on, mC, dxm, dym, dzm);
+    frank3_local(K3, mC, dxm, dym, dzm, px, py, pzC, dfC);
+    sig[0 * SigShape::CELLS + os] = px.x; sig[1 * SigShape::CELLS + os] = px.y; sig[2 * SigShape::CELLS + os] = px.z;
+    sig[3 * SigShape::CELLS + os] = py.x; sig[4 * SigShape::CELLS + os] = py.y; sig[5 * SigShape::CELLS + os] = py.z;
+    if (hn >= 0) {
+      V3<T> hm, hdx = zero, hdy = zero, hdz = zero, hx, hy, hz, hd;
+      if (plate) hm = lds3<T, 2>(pc, hn);
+      else grad_staged(pzm, pc, pzp, hn, hm, hdx, hdy, hdz);
+      frank3_local(K3, hm, hdx, hdy, hdz, hx, hy, hz, hd);
+      const V3<T> sh = hcol == 0 ? hx : hy;
+      sig[0 * SigShape::CELLS + hs] = sh.x;
+      sig[1 * SigShape::CELLS + hs] = sh.y;
+      sig[2 * SigShape::CELLS + hs] = sh.z;
+    }
+    V3<T> uC = zero;
+    if (flow) uC = lds3<T, 2>(su + (p & 3) * S::ELEMS, on);
+    // the director's rate at plane p-1: its pi_x. / pi_y. plane was written one iteration ago
+    if (p > z0) {
+      const T* sg = ssig + ((p - 1) & 1) * SigShape::ELEMS + os;
+      constexpr int CS = SigShape::CELLS, PXs = SigShape::PX;
+      V3<T> h;
+      h.x = T(0.5) * ((sg[0 * CS + 1] - sg[0 * CS - 1]) + (sg[3 * CS + PXs] - sg[3 * CS - PXs]) + (pzC.x - pzA.x)) - dfB.x;
+      h.y = T(0.5) * ((sg[1 * CS + 1] - sg[1 * CS - 1]) + (sg[4 * CS + PXs] - sg[4 * CS - PXs]) + (pzC.y - pzA.y)) - dfB.y;
+      h.z = T(0.5) * ((sg[2 * CS + 1] - sg[2 * CS - 1]) + (sg[5 * CS + PXs] - sg[5 * CS - PXs]) + (pzC.z - pzA.z)) - dfB.z;
+      h.z += C.W0 * mB.z;
+      const T* pm1 = sn + ((p - 1) & 3) * S::ELEMS;            // staged plane p-1 of m
+      const V3<T> gxm = T(0.5) * (lds3<T, 2>(pm1, on + 1) - lds3<T, 2>(pm1, on - 1));
+      const V3<T> gym = T(0.5) * (lds3<T, 2>(pm1, on + S::RS) - lds3<T, 2>(pm1, on - S::RS));
+      const V3<T> gzm = T(0.5) * (mC - mA);
+      V3<T> gxu = zero, gyu = zero, gzu = zero;
+      if (flow) {
+        const T* pu1 = su + ((p - 1) & 3) * S::ELEMS;
+        gxu = T(0.5) * (lds3<T, 2>(pu1, on + 1) - lds3<T, 2>(pu1, on - 1));
+        gyu = T(0.5) * (lds3<T, 2>(pu1, on + S::RS) - lds3<T, 2>(pu1, on - S::RS));
+        gzu = T(0.5) * (uC - uA);
+      }
+      const V3<T> kk = director_rhs_tail(C, C.inv_gamma1 * h, mB, gxm, gym, gzm, uB, gxu, gyu, gzu);
+      if (active) {
+        const unsigned cm = c - G.plane;
+        if (STAGE == 0) {
+          const V3<T> v = unit_fast(mB + C.dt * kk);
+          const V3<T> a = mB + hdt * kk;
+          out_m[cm] = v.x; out_m[cm + N] = v.y; out_m[cm + 2 * N] = v.z;
+          a_out[cm] = a.x; a_out[cm + N] = a.y; a_out[cm + 2 * N] = a.z;
+        } else {
+          const V3<T> a = {a_in[cm], a_in[cm + N], a_in[cm + 2 * N]};
+          const V3<T> v = unit_fast(a + hdt * kk);
+          out_m[cm] = v.x; out_m[cm + N] = v.y; out_m[cm + 2 * N] = v.z;
+        }
+      }
+    }
+    pzA = pzB; pzB = pzC; dfB = dfC;
+    mA = mB; mB = mC; uA = uB; uB = uC;
+    c += G.plane;
+  }
+  cp_async_wait_all();
+}
+
 }  // namespace nh

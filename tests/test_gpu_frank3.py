@@ -25,10 +25,11 @@ def rel_linf(a, b):
     return np.abs(a - b).max() / max(np.abs(b).max(), 1e-300)
 
 
-def check(p, d, steps, label):
+def check(p, d, steps, label, options=0):
     for precision, tu, tn in ((0, FP64_TOL, FP64_TOL), (1, FP32_TOL_U, FP32_TOL_N)):
         o = Oracle(**dict(p, precision=precision))
         g = nh().Lattice(**dict(p, precision=precision))
+        g.set_options(options)
         o.set_director(d)
         g.set_director(d)
         f0o, f0g = o.get_fields(), g.get_fields()
@@ -49,6 +50,7 @@ def test_config0_three_constants(r):
     d = p.pop("director")
     p.pop("steps")
     check(p, d, 100, "frank3 cfg0 r=%d" % r)
+    check(p, d, 100, "frank3 cfg0 r=%d, one thread per cell" % r, options=nh().OPT_FD_DIRECT)
 
 
 def test_skyrmion_tube_three_constants():
@@ -66,6 +68,7 @@ def test_three_constants_with_viscous_stress_free_plates_and_W0():
     p = dict(nx=nx, ny=ny, nz=nz, tau=0.7, K3=K3, pitch=9.0, xi=1.0946, gamma1=0.4293, g=(2e-6, -1e-6, 0.0),
              fd_ratio=2, alpha=tuple(0.1 * a for a in MBBA), anchoring=1, W0=1e-3)
     check(p, d, 40, "frank3 + visc + free plates")
+    check(p, d, 40, "frank3 + visc + free plates, one thread per cell", options=nh().OPT_FD_DIRECT)
     for shape in ((1, 1, 3), (17, 5, 6)):
         nx, ny, nz = shape
         q = dict(p, nx=nx, ny=ny, nz=nz, anchoring=0)
