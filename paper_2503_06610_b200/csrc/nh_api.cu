@@ -444,7 +444,19 @@ int launch_force(nh_lattice* L) {
     br.end();
     const bool tiled3 = !(L->options & NH_OPT_FD_DIRECT) && tiles_fit(L);
     // h (through pi) is needed by the viscous stress, and by the one-thread-per-cell form always
-    if (C.visc || !tiled3) { const int rc = launch_h3<T>(L, n, KC_FORCE); if (rc) return rc; }
+    if (C.visc && tiled3) {
+      Bracket bh(L, KC_FORCE);
+      if (bh.rc) return bh.rc;
+      const TileGrid g = tile_grid(L);
+      const size_t sm = nh::force_smem_bytes<T, true>();
+      if (tiles_vec(L))
+        nh::director3_tile_kernel<T, 2, true><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(
+            n, u, nullptr, (T*)L->h3, nullptr, L->G, C, frank3_const<T>(L), 0, g.zchunk);
+      else
+        nh::director3_tile_kernel<T, 2, false><<<g.grid, nh::TILE_THREADS, sm, L->stream>>>(
+            n, u, nullptr, (T*)L->h3, nullptr, L->G, C, frank3_const<T>(L), 0, g.zchunk);
+      bh.end();
+    } else if (!tiled3) { const int rc = launch_h3<T>(L, n, KC_FORCE); if (rc) return rc; }
     Bracket b3(L, KC_FORCE);
     if (b3.rc) return b3.rc;
     if (tiled3) {
@@ -603,6 +615,8 @@ int enable_tile_smem() {
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false, false>, attr, fb));
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, true, true>, attr, fvb));
   NH_CUDA(cudaFuncSetAttribute(nh::force_tile_kernel<T, false, true>, attr, fvb));
+  NH_CUDA(cudaFuncSetAttribute(nh::director3_tile_kernel<T, 2, true>, attr, fvb));
+  NH_CUDA(cudaFuncSetAttribute(nh::director3_tile_kernel<T, 2, false>, attr, fvb));
   NH_CUDA(cudaFuncSetAttribute(nh::director3_tile_kernel<T, 0, true>, attr, fvb));
   NH_CUDA(cudaFuncSetAttribute(nh::director3_tile_kernel<T, 1, true>, attr, fvb));
   NH_CUDA(cudaFuncSetAttribute(nh::director3_tile_kernel<T, 0, false>, attr, fvb));

@@ -454,6 +454,7 @@ force_tile_kernel(const T* __restrict__ n, const T* __restrict__ u, T* __restric
 // projection shared with the one-constant path).  The own cell's column of m and u is carried in
 // registers (plane p-2 is being overwritten in the ring by then).
 //   STAGE 0: out_m = n^P = unit(m + dt k1), a_out = m + dt/2 k1;  STAGE 1: out_m = unit(a_in + dt/2 k2)
+//   STAGE 2: out_m = h itself (for N of the viscous stress in the force kernel)
 template <typename T, int STAGE, bool VEC>
 __global__ void __launch_bounds__(TILE_THREADS)
 director3_tile_kernel(const T* __restrict__ m, const T* __restrict__ u, const T* __restrict__ a_in,
@@ -561,10 +562,13 @@ director3_tile_kernel(const T* __restrict__ m, const T* __restrict__ u, const T*
         gyu = T(0.5) * (lds3<T, 2>(pu1, on + S::RS) - lds3<T, 2>(pu1, on - S::RS));
         gzu = T(0.5) * (uC - uA);
       }
-      const V3<T> kk = director_rhs_tail(C, C.inv_gamma1 * h, mB, gxm, gym, gzm, uB, gxu, gyu, gzu);
+      V3<T> kk = zero;
+      if (STAGE != 2) kk = director_rhs_tail(C, C.inv_gamma1 * h, mB, gxm, gym, gzm, uB, gxu, gyu, gzu);
       if (active) {
         const unsigned cm = c - G.plane;
-        if (STAGE == 0) {
+        if (STAGE == 2) {
+          out_m[cm] = h.x; out_m[cm + N] = h.y; out_m[cm + 2 * N] = h.z;
+        } else if (STAGE == 0) {
           const V3<T> v = unit_fast(mB + C.dt * kk);
           const V3<T> a = mB + hdt * kk;
           out_m[cm] = v.x; out_m[cm + N] = v.y; out_m[cm + 2 * N] = v.z;
