@@ -36,7 +36,8 @@ def parse():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index; 5 = the paper's 320x320x16 "
+                    "many-skyrmion demonstration (PAPER.md:284) on its test-case material, Delta t_FD = 250")
     ap.add_argument("--precision", default="fp32s", choices=sorted(PRECISIONS))
     ap.add_argument("--size", type=int, nargs=3, default=None, help="configs[4] grid (nx ny nz)")
     ap.add_argument("--options", type=lambda v: int(v, 0), default=0, help="nh_set_options bits (kernel variants)")
@@ -60,7 +61,7 @@ def workload(args):
         over["size"] = tuple(args.size)
     if args.fd_ratio is not None:
         over["fd_ratio"] = args.fd_ratio
-    p = I.config(args.config, **over)
+    p = I.many_skyrmions(**over) if args.config == 5 else I.config(args.config, **over)
     if args.leslie:
         # alpha1..alpha6 of MBBA in simulation units as printed in the paper's Table 1
         table1 = (0.0373, -0.4496, -0.0203, 0.9318, 0.3084, -0.1617)
@@ -68,16 +69,19 @@ def workload(args):
     if args.frank3:
         # K11 : K22 : K33 = 1.67 : 0.788 : 2.62
         p["K3"] = (p["K"], p["K"] * 0.788 / 1.67, p["K"] * 2.62 / 1.67)
+    if args.leslie and args.config == 5:
+        p["alpha"] = tuple(args.leslie * a for a in I.MBBA_ALPHA)
     d = p.pop("director")
     p.pop("steps")
     name = {0: "configs[0] tiny channel", 1: "configs[1] single skyrmion tube", 2: "configs[2] precision sweep domain",
-            3: "configs[3] two skyrmion tubes in Poiseuille flow", 4: "configs[4] skyrmion lattice"}[args.config]
+            3: "configs[3] two skyrmion tubes in Poiseuille flow", 4: "configs[4] skyrmion lattice",
+            5: "many-skyrmion demonstration (PAPER.md:284), 20 tubes, free plates, W0"}[args.config]
     desc = {"workload": "%s %dx%dx%d" % (name, p["nx"], p["ny"], p["nz"]), "grid": [p["nx"], p["ny"], p["nz"]],
-            "fd_ratio": p["fd_ratio"], "tau": p["tau"], "K": p["K"], "pitch": p["pitch"], "xi": p["xi"],
+            "fd_ratio": p["fd_ratio"], "tau": p["tau"], "K": p.get("K", 0.0), "pitch": p["pitch"], "xi": p["xi"],
             "g_x": p["g"][0], "precision": args.precision}
     if args.leslie:
         desc["leslie_viscous_stress"] = "Table 1 x %g" % args.leslie
-    if args.frank3:
+    if args.frank3 or args.config == 5:
         desc["frank_constants"] = list(p["K3"])
     return p, d, desc
 

@@ -129,6 +129,54 @@ def lattice_centres(nx: int, ny: int, spacing: float = 48.0, jitter: float = 6.0
     return out
 
 
+def random_centres(nx: int, ny: int, count: int, min_dist: float, seed: int = SEED):
+    """`count` tube centres drawn uniformly on the periodic nx x ny plane, a draw being rejected when it
+    falls within `min_dist` (periodic minimum image) of an accepted one: "randomly placed skyrmions"
+     that do not overlap.  Counter-based draws, so the list depends on the seed only."""
+    out, k = [], 0
+    while len(out) < count:
+        if k > 10000 * count:
+            raise ValueError("cannot place %d centres %g apart on %dx%d" % (count, min_dist, nx, ny))
+        c = np.array([k], dtype=np.uint64)
+        x = uniform01(seed + 3, c, 0)[0] * nx
+        y = uniform01(seed + 3, c, 1)[0] * ny
+        k += 1
+        ok = True
+        for (xa, ya) in out:
+            dx, dy = x - xa, y - ya
+            dx -= nx * round(dx / nx)
+            dy -= ny * round(dy / ny)
+            if dx * dx + dy * dy < min_dist * min_dist:
+                ok = False
+                break
+        if ok:
+            out.append((float(x), float(y)))
+    return out
+
+
+# alpha1..alpha6 of MBBA in simulation units as the paper's Table 1 prints them (PAPER.md:168-185;
+# tests/golden/table1_mbba.txt holds the same numbers with the citation)
+MBBA_ALPHA = (0.0373, -0.4496, -0.0203, 0.9318, 0.3084, -0.1617)
+MBBA_K3 = (1.67e-7, 7.88e-8, 2.62e-7)
+
+
+def many_skyrmions(nx: int = 320, ny: int = 320, nz: int = 16, count: int = 20, **over) -> dict:
+    """The paper's closing demonstration (Fig. 6): a 320x320x16 cell with 20 randomly placed
+    skyrmions, single precision, Delta t_FD = 250, on the test case's material (MBBA's
+    three Frank constants, pitch 14, free plates, W0 = 1.5e-8, g = 2e-9; gamma1, xi from Table 1 with
+    Parodi's relation).  Stand-in: the tubes are this module's ansatz, not the ref.-[18] toron
+    (out of scope); elastic stress only unless ``alpha`` is given (the explicit viscous force is
+    unstable at this Delta t_FD)."""
+    gamma1 = MBBA_ALPHA[2] - MBBA_ALPHA[1]
+    xi = -(MBBA_ALPHA[2] + MBBA_ALPHA[1]) / gamma1
+    p = dict(nx=nx, ny=ny, nz=nz, tau=1.0, K3=MBBA_K3, pitch=14.0, xi=xi, gamma1=gamma1,
+             g=(2e-9, 0.0, 0.0), anchoring=1, W0=1.5e-8, fd_ratio=250, steps=1000)
+    p.update(over)
+    seed = p.pop("seed", SEED)
+    p["director"] = skyrmion_tubes(nx, ny, nz, random_centres(nx, ny, count, 2.0 * 7.0 + 4.0, seed), 7.0)
+    return p
+
+
 def config(k: int, **over) -> dict:
     """Parameter set + director for BASELINE.json ``configs[k]`` (k = 0..4).
 
