@@ -49,6 +49,11 @@ def parse():
     ap.add_argument("--fd-ratio", type=int, default=None, help="override the config's Delta t_FD / Delta t_LB")
     ap.add_argument("--frank3", action="store_true",
                     help="three-constant Frank energy (row f2): K11 = K, K22 : K33 in the ratios of the paper's Table 1")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="row f4: ONE lattice cut into y-slabs with halo exchange (paper_2503_06610_b200/slabs.py) instead of "
+                         "independent replicas.  Under torchrun: one slab per rank over NCCL, the config's ny rows PER RANK "
+                         "(weak scaling; the value is ignored).  On one GPU: the config's lattice cut into this many slabs "
+                         "held by one process (measures the decomposition's overhead)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -227,6 +232,66 @@ def job_mlups(world, fluid_cells, lb_steps, ms):
     return world * fluid_cells * lb_steps / (ms * 1e-3) / 1e6
 
 
+def run_slabs(args, world, rank, local):
+    """One lattice cut along y (SURVEY.md section 8e).  N > 1: the global lattice has world x ny rows, rank s holds slab s;
+    N = 1: the config's own lattice in args.slabs slabs on this device.  Same timing rules as the main line."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import paper_2503_06610_b200 as nh
+    from paper_2503_06610_b200.slabs import SlabLattice
+
+    p, d, desc = workload(args)
+    prec = PRECISIONS[args.precision]
+    r = max(1, p["fd_ratio"])
+    if world > 1:
+        d = np.concatenate([d] * world, axis=2)          # the config's director tiled along y: still periodic
+        p = dict(p, ny=p["ny"] * world)
+    nslabs = world if world > 1 else args.slabs
+    nf = p["nx"] * p["ny"] * (p["nz"] - 2)
+    lat = SlabLattice(slabs=nslabs, group=dist.group.WORLD if world > 1 else None, device="cuda:%d" % local,
+                      **dict(p, precision=prec))
+    lat.set_director(d)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        lat.step(r)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = sum(x.launch_count for x in lat.local.values())
+    x0, b0 = lat.exchanges, lat.bytes_sent
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        lat.step(r)
+    ev1.record()
+    barrier()
+    ms = max_over_ranks(ev0.elapsed_time(ev1), world)
+    launches = sum(x.launch_count for x in lat.local.values()) - l0
+    clocks = sampler.stop() if rank == 0 else None
+    if rank == 0:
+        line = {"metric": METRIC, "value": nf * r * args.steps / (ms * 1e-3) / 1e6, "unit": "MLUPS", "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": DTYPE[prec], "data": "synthetic",
+                "config": dict(desc, grid=[p["nx"], p["ny"], p["nz"]], lb_steps_per_step=r, fluid_cells=nf,
+                               parallelism="y-slabs x%d, halo %d rows%s" % (nslabs, lat.H, "" if world > 1 else " (one device)"),
+                               exchanges_per_step=(lat.exchanges - x0) / args.steps,
+                               halo_bytes_sent_per_step_per_process=(lat.bytes_sent - b0) / args.steps),
+                "clocks": clocks, "gpu_launches": launches, "roofline": None}
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     args = parse()
     if args.impl == "reference":
@@ -249,6 +314,9 @@ def main():
         nh_build.build()
     if world > 1:
         dist.barrier()
+
+    if args.slabs:
+        return run_slabs(args, world, rank, local)
 
     p, d, desc = workload(args)
     prec = PRECISIONS[args.precision]

@@ -156,6 +156,38 @@ int nh_set_options(nh_lattice* L, int options);
  *        4 = force, 5 = everything else (conversions, initialisation), 6 = two-step LB launches. */
 int nh_kernel_time(nh_lattice* L, int which, double* ms_total, long* launches);
 
+/* ---- Slab decomposition along y (the paper's own runs are single-GPU,
+ * PAPER.md:284).  A rank's lattice holds its rows plus H halo rows on either side; its periodic wrap in y
+ * then only feeds the outermost halo rows, and every operator eats into the valid halo by its stencil
+ * radius, so the halos are refreshed from the neighbours between calls with the two
+ * copies below.  Both are asynchronous on the lattice's stream and touch no other state.
+ *
+ * nh_get_rows: pack rows [y0, y0 + nrows) of one field -- all x, ALL z (plate layers included), all
+ * components -- into the contiguous DEVICE buffer `dev_buf`, laid out [component][z][row][x] in the
+ * lattice's storage type (4 or 8 bytes per word; nh_rows_bytes gives the size).  nh_set_rows is the inverse.
+ * field: NH_FIELD_POPULATIONS  the 19 post-collision populations the next LB step gathers from
+ *        NH_FIELD_DIRECTOR     the current director n (3 components)
+ *        NH_FIELD_VELOCITY     u as stored by the last director update (3)
+ *        NH_FIELD_FORCE        F^LC (3)
+ * NH_EINVAL for a null handle or buffer, an unknown field, or rows outside [0, ny). */
+#define NH_FIELD_POPULATIONS 0
+#define NH_FIELD_DIRECTOR    1
+#define NH_FIELD_VELOCITY    2
+#define NH_FIELD_FORCE       3
+size_t nh_rows_bytes(const nh_lattice* L, int field, int nrows);
+int nh_get_rows(nh_lattice* L, int field, int y0, int nrows, void* dev_buf);
+int nh_set_rows(nh_lattice* L, int field, int y0, int nrows, const void* dev_buf);
+
+/* Recompute F^LC (Eq. 12) from the director and the stored velocity now in the lattice -- the force
+ * step of nh_step on its own, for use after the director's (and, with Leslie viscosities, the
+ * velocity's) halo rows have been refreshed.  Asynchronous on the lattice's stream. */
+int nh_update_force(nh_lattice* L);
+
+/* on != 0: nh_step no longer recomputes F^LC after a director update; the caller owes an nh_update_force
+ * before the next LB step (the slab driver refreshes the director's halo rows in between, so the force
+ * computed inside nh_step would be thrown away).  Graph replay is bypassed while this is on.  Default 0. */
+int nh_defer_force(nh_lattice* L, int on);
+
 void nh_free(nh_lattice* L);
 const char* nh_last_error(void);
 

@@ -20,7 +20,8 @@ OPT_LB_ONESTEP, OPT_LB_BLOCKORDER = 128, 1 << 26
 KERNEL_CLASSES = ("lb", "velocity", "predictor", "corrector", "force", "other", "lb2")
 
 EXPORTS = ("nh_workspace_bytes", "nh_init_lattice", "nh_set_director", "nh_step", "nh_get_fields",
-           "nh_time", "nh_launch_count", "nh_set_options", "nh_kernel_time", "nh_free", "nh_last_error")
+           "nh_time", "nh_launch_count", "nh_set_options", "nh_kernel_time", "nh_free", "nh_last_error",
+           "nh_rows_bytes", "nh_get_rows", "nh_set_rows", "nh_update_force", "nh_defer_force")
 
 
 class NhParams(C.Structure):
@@ -30,6 +31,9 @@ class NhParams(C.Structure):
                 ("anchoring", C.c_int), ("W0", C.c_double), ("fd_ratio", C.c_int),
                 ("precision", C.c_int), ("coupling", C.c_int), ("alpha", C.c_double * 6),
                 ("K3", C.c_double * 3)]
+
+
+FIELDS = ("populations", "director", "velocity", "force")   # NH_FIELD_* of include/nh.h, in order
 
 
 class NhError(RuntimeError):
@@ -63,6 +67,12 @@ def load():
         lib.nh_launch_count.restype = C.c_long
         lib.nh_set_options.argtypes = [C.c_void_p, C.c_int]
         lib.nh_kernel_time.argtypes = [C.c_void_p, C.c_int, dp, C.POINTER(C.c_long)]
+        lib.nh_rows_bytes.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        lib.nh_rows_bytes.restype = C.c_size_t
+        lib.nh_get_rows.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
+        lib.nh_set_rows.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
+        lib.nh_update_force.argtypes = [C.c_void_p]
+        lib.nh_defer_force.argtypes = [C.c_void_p, C.c_int]
         lib.nh_free.argtypes = [C.c_void_p]
         lib.nh_free.restype = None
         lib.nh_last_error.restype = C.c_char_p
@@ -167,3 +177,26 @@ class Lattice:
 
     def synchronize(self):
         self._stream.synchronize()
+
+    # ---- halo rows of a y-slab (include/nh.h, "Slab decomposition along y") ----
+    def rows_bytes(self, field, nrows):
+        return int(load().nh_rows_bytes(self._h, FIELDS.index(field), int(nrows)))
+
+    def new_rows_buffer(self, field, nrows):
+        """Device buffer that holds `nrows` packed rows of `field` ([component][z][row][x], storage type)."""
+        import torch
+        return torch.empty(self.rows_bytes(field, nrows), dtype=torch.uint8, device=self.device)
+
+    def get_rows(self, field, y0, nrows, buf):
+        assert buf.is_cuda and buf.is_contiguous() and buf.numel() * buf.element_size() >= self.rows_bytes(field, nrows)
+        _check(load().nh_get_rows(self._h, FIELDS.index(field), int(y0), int(nrows), buf.data_ptr()))
+
+    def set_rows(self, field, y0, nrows, buf):
+        assert buf.is_cuda and buf.is_contiguous() and buf.numel() * buf.element_size() >= self.rows_bytes(field, nrows)
+        _check(load().nh_set_rows(self._h, FIELDS.index(field), int(y0), int(nrows), buf.data_ptr()))
+
+    def update_force(self):
+        _check(load().nh_update_force(self._h))
+
+    def defer_force(self, on=True):
+        _check(load().nh_defer_force(self._h, 1 if on else 0))

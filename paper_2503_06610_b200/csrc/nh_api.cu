@@ -107,6 +107,7 @@ struct nh_lattice {
   unsigned order_len;
   int order_key;                   // (D << 8) | nzf the tables were built for, -1: none
   int sm_count;
+  int defer_force;                 // nh_defer_force: nh_step leaves F^LC to a later nh_update_force
   // CUDA-graph replay of nh_step (NH_OPT_GRAPH): one executable graph per distinct call shape
   struct Graph {
     int n_lb, r, phase, cur, ncur, sweep, options;   // key: arguments and the state the launches depend on
@@ -648,7 +649,7 @@ int step_typed(nh_lattice* L, int n_lb, int r) {
       // u(t): for the director equation (coupling bit1) and for the viscous stress in the force
       if ((L->p.coupling & 2) || viscous(L)) { rc = launch_velocity<T, SH>(L); if (rc) return rc; }
       rc = launch_director<T>(L, r); if (rc) return rc;
-      rc = launch_force<T>(L); if (rc) return rc;
+      if (!L->defer_force) { rc = launch_force<T>(L); if (rc) return rc; }
     }
   }
   NH_CUDA(cudaGetLastError());
@@ -802,6 +803,59 @@ int step_graph(nh_lattice* L, int n_lb, int r) {
 
 }  // namespace
 
+namespace {
+
+// rows [y0, y0 + nrows) of a [comps][nz][ny][nx] field <-> a contiguous [comps][nz][nrows][nx] buffer
+template <typename T, bool PACK>
+__global__ void rows_kernel(T* __restrict__ field, T* __restrict__ buf, nh::Geom G, int y0, int nrows) {
+  // blockIdx.y = component * nz + z; the block's threads run along the nrows * nx contiguous words of that plane
+  const unsigned per = (unsigned)nrows * G.nx;
+  const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= per) return;
+  const unsigned c = blockIdx.y / G.nz, z = blockIdx.y - c * G.nz;
+  const size_t at = (size_t)c * G.N + (size_t)z * G.plane + (size_t)y0 * G.nx + i;   // rows y0.. are contiguous in a plane
+  const size_t to = (size_t)blockIdx.y * per + i;
+  if (PACK) buf[to] = field[at];
+  else field[at] = buf[to];
+}
+
+int field_of(nh_lattice* L, int field, void** base, int* comps) {
+  switch (field) {
+    case NH_FIELD_POPULATIONS: *base = L->f[L->cur]; *comps = 19; return NH_OK;
+    case NH_FIELD_DIRECTOR: *base = L->n[L->ncur]; *comps = 3; return NH_OK;
+    case NH_FIELD_VELOCITY: *base = L->u; *comps = 3; return NH_OK;
+    case NH_FIELD_FORCE: *base = L->F; *comps = 3; return NH_OK;
+    default: return fail(NH_EINVAL, "unknown field");
+  }
+}
+
+template <typename T, bool PACK>
+int rows_typed(nh_lattice* L, int field, int y0, int nrows, void* buf) {
+  void* base = nullptr;
+  int comps = 0;
+  const int rc = field_of(L, field, &base, &comps);
+  if (rc) return rc;
+  const size_t total = (size_t)comps * L->G.nz * nrows * L->G.nx;
+  if (total == 0) return NH_OK;
+  Bracket br(L, KC_OTHER);
+  const dim3 grid(blocks_for((size_t)nrows * L->G.nx), (unsigned)(comps * L->G.nz));
+  rows_kernel<T, PACK><<<grid, BLOCK, 0, L->stream>>>((T*)base, (T*)buf, L->G, y0, nrows);
+  br.end();
+  NH_CUDA(cudaGetLastError());
+  return NH_OK;
+}
+
+int rows_check(nh_lattice* L, int y0, int nrows, const void* buf) {
+  if (!L) return fail(NH_EINVAL, "null handle");
+  if (!buf) return fail(NH_EINVAL, "null buffer");
+  if (nrows < 0 || y0 < 0 || (long)y0 + nrows > L->G.ny) return fail(NH_EINVAL, "rows outside [0, ny)");
+  return NH_OK;
+}
+
+bool is_f32(const nh_lattice* L) { return L->p.precision == NH_FP32_SHIFTED || L->p.precision == NH_FP32_UNSHIFTED; }
+
+}  // namespace
+
 extern "C" {
 
 const char* nh_last_error(void) { return g_err.c_str(); }
@@ -905,7 +959,7 @@ int nh_step(nh_lattice* L, int n_lb, int n_fd) {
   if (!L) return fail(NH_EINVAL, "null handle");
   if (n_lb < 0) return fail(NH_EINVAL, "n_lb must be >= 0");
   const int r = n_fd < 0 ? L->p.fd_ratio : n_fd;
-  if ((L->options & NH_OPT_GRAPH) && n_lb > 0) {
+  if ((L->options & NH_OPT_GRAPH) && n_lb > 0 && !L->defer_force) {
     const int rc = step_graph(L, n_lb, r);
     if (rc != NH_EAGAIN) return rc;          // the stream cannot be captured: plain launches
   }
@@ -918,6 +972,40 @@ int nh_get_fields(nh_lattice* L, double* rho, double* u, double* n, double* F_lc
               (get_fields_typed<float, true>(L, rho, u, n, F_lc)),
               (get_fields_typed<float, false>(L, rho, u, n, F_lc)),
               (get_fields_typed<double, false>(L, rho, u, n, F_lc)));
+}
+
+size_t nh_rows_bytes(const nh_lattice* L, int field, int nrows) {
+  if (!L || nrows < 0 || field < NH_FIELD_POPULATIONS || field > NH_FIELD_FORCE) return 0;
+  const size_t comps = field == NH_FIELD_POPULATIONS ? 19 : 3;
+  return comps * L->G.nz * (size_t)nrows * L->G.nx * (is_f32(L) ? 4 : 8);
+}
+
+int nh_get_rows(nh_lattice* L, int field, int y0, int nrows, void* dev_buf) {
+  const int rc = rows_check(L, y0, nrows, dev_buf);
+  if (rc) return rc;
+  return is_f32(L) ? rows_typed<float, true>(L, field, y0, nrows, dev_buf)
+                   : rows_typed<double, true>(L, field, y0, nrows, dev_buf);
+}
+
+int nh_set_rows(nh_lattice* L, int field, int y0, int nrows, const void* dev_buf) {
+  const int rc = rows_check(L, y0, nrows, dev_buf);
+  if (rc) return rc;
+  return is_f32(L) ? rows_typed<float, false>(L, field, y0, nrows, const_cast<void*>(dev_buf))
+                   : rows_typed<double, false>(L, field, y0, nrows, const_cast<void*>(dev_buf));
+}
+
+int nh_defer_force(nh_lattice* L, int on) {
+  if (!L) return fail(NH_EINVAL, "null handle");
+  L->defer_force = on ? 1 : 0;
+  return NH_OK;
+}
+
+int nh_update_force(nh_lattice* L) {
+  if (!L) return fail(NH_EINVAL, "null handle");
+  const int rc = is_f32(L) ? launch_force<float>(L) : launch_force<double>(L);
+  if (rc) return rc;
+  NH_CUDA(cudaGetLastError());
+  return NH_OK;
 }
 
 long nh_time(const nh_lattice* L) { return L ? L->t : -1; }

@@ -57,6 +57,15 @@ def test_workspace_bytes_and_validation(lib):
     assert nh.workspace_bytes(nh.make_params(512, 512, 128, 0.8)) < 8 * 2 ** 30  # BASELINE: "roughly 7 GB"
 
 
+def test_slab_calls_reject_null_handles(lib):
+    lib.nh_rows_bytes.restype = C.c_size_t
+    assert lib.nh_rows_bytes(None, 0, 4) == 0
+    assert lib.nh_get_rows(None, 0, 0, 1, 256) == -1 and lib.nh_last_error()
+    assert lib.nh_set_rows(None, 0, 0, 1, 256) == -1
+    assert lib.nh_update_force(None) == -1
+    assert lib.nh_defer_force(None, 1) == -1
+
+
 def test_null_and_small_workspace(lib):
     p = nh.make_params(4, 4, 5, 0.8)
     h = C.c_void_p()

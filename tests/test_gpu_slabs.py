@@ -1,0 +1,189 @@
+"""Slab decomposition along y on the GPU, through the C ABI: the lattice cut
+into 1, 2, 3 slabs held by ONE process on ONE device (the slabs are advanced one after the other; nothing on
+the device waits for anything else) must give, bit for bit, the fields of the undivided lattice -- same
+kernels, same neighbour values -- and so agrees with the oracle to the same tolerance.  The exchange between
+processes (NCCL / gloo point-to-point) is the same code path with the copies replaced by isend/irecv; its
+host logic is covered on the CPU by tests/test_slabs_host.py."""
+import numpy as np
+import pytest
+
+import nh_inputs as I
+from oracle import Oracle
+
+pytestmark = pytest.mark.gpu
+
+MBBA = I.MBBA_ALPHA
+MODELS = {
+    "one-constant": dict(K=0.01, pitch=16.0, xi=0.6, gamma1=1.0),
+    "leslie": dict(K=0.01, pitch=16.0, xi=0.6, gamma1=1.0, alpha=tuple(0.1 * a for a in MBBA)),
+    "full model": dict(K3=(0.01, 0.005, 0.015), pitch=16.0, xi=1.09, gamma1=0.43, alpha=tuple(0.1 * a for a in MBBA),
+                       anchoring=1, W0=1e-3),
+}
+
+
+def _lib():
+    import paper_2503_06610_b200 as nh
+    from paper_2503_06610_b200 import build
+    build.build()
+    return nh
+
+
+def _run(obj, d, chunks):
+    obj.set_director(d)
+    for c in chunks:
+        obj.step(c)
+
+
+@pytest.mark.parametrize("model", sorted(MODELS))
+@pytest.mark.parametrize("precision", ["fp64", "fp32s"])
+def test_cut_lattice_is_bit_identical_and_matches_the_oracle(model, precision):
+    nh = _lib()
+    from paper_2503_06610_b200.slabs import SlabLattice
+    prec = {"fp64": nh.FP64_SHIFTED, "fp32s": nh.FP32_SHIFTED}[precision]
+    nx, ny, nz, r, chunks = 24, 46, 10, 4, (1, 6, 9, 8)
+    base = dict(nx=nx, ny=ny, nz=nz, tau=0.9, g=(1e-6, 0.0, 0.0), fd_ratio=r, **MODELS[model])
+    d = I.skyrmion_tubes(nx, ny, nz, [(11.0, 20.0)], 8.0)
+    whole = nh.Lattice(**dict(base, precision=prec))
+    _run(whole, d, chunks)
+    ref = whole.get_fields()
+    whole.close()
+    for slabs in (1, 2, 3):
+        s = SlabLattice(slabs=slabs, **dict(base, precision=prec))
+        _run(s, d, chunks)
+        got = s.gather_fields()
+        assert s.time == sum(chunks) and s.exchanges > 0
+        s.close()
+        for k in ("rho", "u", "n", "F"):
+            assert np.array_equal(got[k], ref[k]), (model, precision, slabs, k, np.abs(got[k] - ref[k]).max())
+    o = Oracle(**dict(base, precision=0))
+    _run(o, d, chunks)
+    fo = o.get_fields()
+    tol_u, tol_n = (1e-10, 1e-10) if precision == "fp64" else (1e-3, 1e-4)
+    assert np.abs(ref["u"] - fo["u"]).max() / np.abs(fo["u"]).max() <= tol_u
+    assert np.abs(ref["n"] - fo["n"]).max() <= tol_n
+
+
+def test_slabs_wide_enough_for_the_two_step_kernel():
+    """Slabs of 264 x 256 cells per plane run the two-step LB kernel (lb2_usable); the whole 512-row lattice runs
+    it in two strips: still bit-identical, and the two-step launches really happen on the slabs."""
+    nh = _lib()
+    from paper_2503_06610_b200.slabs import SlabLattice
+    nx, ny, nz, r = 256, 512, 18, 10
+    base = dict(nx=nx, ny=ny, nz=nz, tau=0.8, K=0.01, pitch=32.0, xi=0.5, gamma1=1.0, g=(1e-6, 0.0, 0.0),
+                fd_ratio=r, precision=nh.FP32_SHIFTED)
+    d = I.skyrmion_tubes(nx, ny, nz, I.lattice_centres(nx, ny), 16.0)
+    whole = nh.Lattice(**base)
+    _run(whole, d, (25,))
+    ref = whole.get_fields(which=("u", "n"))
+    whole.close()
+    s = SlabLattice(slabs=2, **base)
+    for lat in s.local.values():
+        lat.set_options(nh.OPT_TIMING)
+    _run(s, d, (25,))
+    got = s.gather_fields(which=("u", "n"))
+    two_step_launches = sum(lat.kernel_time("lb2")[1] for lat in s.local.values())
+    s.close()
+    assert two_step_launches > 0
+    assert np.array_equal(got["u"], ref["u"]) and np.array_equal(got["n"], ref["n"])
+
+
+def test_rows_round_trip_and_bad_arguments():
+    nh = _lib()
+    import torch
+    lat = nh.Lattice(nx=8, ny=12, nz=5, tau=0.8, K=0.01, precision=nh.FP64_SHIFTED)
+    d = I.random_unit_field(8, 12, 5)
+    lat.set_director(d)
+    n0 = lat.get_fields(which=("n",))["n"]
+    assert lat.rows_bytes("director", 3) == 3 * 5 * 3 * 8 * 8 and lat.rows_bytes("populations", 2) == 19 * 5 * 2 * 8 * 8
+    buf = lat.new_rows_buffer("director", 3)
+    lat.get_rows("director", 2, 3, buf)
+    lat.synchronize()
+    packed = buf.cpu().numpy().view(np.float64).reshape(3, 5, 3, 8)
+    assert np.array_equal(packed, n0[:, :, 2:5, :])                # layout [component][z][row][x], plates included
+    lat.set_rows("director", 7, 3, buf)                            # rows 2..4 copied onto rows 7..9
+    n1 = lat.get_fields(which=("n",))["n"]
+    assert np.array_equal(n1[:, :, 7:10, :], n0[:, :, 2:5, :]) and np.array_equal(n1[:, :, :7, :], n0[:, :, :7, :])
+    for bad in ((-1, 2), (11, 2), (0, 13)):
+        with pytest.raises(nh.NhError):
+            lat.get_rows("director", bad[0], bad[1], lat.new_rows_buffer("director", 13))
+    lat.close()
+    assert torch.cuda.is_available()
+
+
+def test_an_underestimated_reach_changes_the_answer(monkeypatch):
+    """Negative control on the real kernels: tell the schedule that the director update reads u one row less far
+    than it does, and the cut lattice no longer reproduces the whole one -- the bit-identity above is earned."""
+    nh = _lib()
+    from paper_2503_06610_b200 import slabs as S
+    true_of = S.Reach.of
+    monkeypatch.setattr(S.Reach, "of", staticmethod(lambda **kw: S.Reach(2, 1, 2, 0, True)))
+    assert true_of().fd_velocity == 2
+    nx, ny, nz, r, chunks = 24, 46, 10, 4, (1, 6, 9, 8)
+    base = dict(nx=nx, ny=ny, nz=nz, tau=0.9, g=(1e-6, 0.0, 0.0), fd_ratio=r, precision=nh.FP64_SHIFTED, **MODELS["one-constant"])
+    d = I.skyrmion_tubes(nx, ny, nz, [(11.0, 20.0)], 8.0)
+    whole = nh.Lattice(**base)
+    _run(whole, d, chunks)
+    ref = whole.get_fields(which=("n",))["n"]
+    whole.close()
+    s = S.SlabLattice(slabs=2, halo=3, **base)
+    _run(s, d, chunks)
+    got = s.gather_fields(which=("n",))["n"]
+    s.close()
+    assert not np.array_equal(got, ref)
+
+
+WORKER = r"""
+import os, sys
+sys.path.insert(0, %r); sys.path.insert(0, os.path.join(%r, "tests"))
+import numpy as np
+import torch, torch.distributed as dist
+import nh_inputs as I
+import paper_2503_06610_b200 as nh
+from paper_2503_06610_b200.slabs import SlabLattice
+import test_gpu_slabs as T
+rank = int(os.environ["RANK"])
+torch.cuda.set_device(0)
+dist.init_process_group("gloo", rank=rank, world_size=2)
+nx, ny, nz, r, chunks = 24, 46, 10, 4, (1, 6, 9, 8)
+for model in ("one-constant", "full model"):
+    base = dict(nx=nx, ny=ny, nz=nz, tau=0.9, g=(1e-6, 0.0, 0.0), fd_ratio=r, precision=nh.FP32_SHIFTED, **T.MODELS[model])
+    d = I.skyrmion_tubes(nx, ny, nz, [(11.0, 20.0)], 8.0)
+    whole = nh.Lattice(**base)
+    T._run(whole, d, chunks)
+    ref = whole.get_fields()
+    whole.close()
+    s = SlabLattice(group=dist.group.WORLD, **base)
+    T._run(s, d, chunks)
+    (idx, (y0, rows, f)), = s.get_fields().items()
+    assert idx == rank and rows == 23
+    for k in ref:
+        assert np.array_equal(f[k], ref[k][..., y0:y0 + rows, :]), (model, k)
+    s.close()
+dist.barrier()
+print("rank", rank, "slabs ok")
+dist.destroy_process_group()
+"""
+
+
+def test_two_processes_exchange_halos_of_real_lattices(tmp_path):
+    """The rank-to-rank path (batched isend/irecv, one slab per process) with the real kernels: two processes
+    share the one GPU, each advances its slab on its own and hands its edge rows over through a gloo group
+    (staged in host memory; on several GPUs the same calls go over NCCL).  Each must hold, bit for bit, its
+    rows of the undivided lattice."""
+    import os
+    import subprocess
+    import sys
+    _lib()
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER % (root, root))
+    port = 33500 + os.getpid() % 2000
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.STDOUT, text=True))
+    outs = [p.communicate(timeout=600)[0] for p in procs]
+    for rank, (p, o) in enumerate(zip(procs, outs)):
+        assert p.returncode == 0, o
+        assert "rank %d slabs ok" % rank in o
