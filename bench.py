@@ -43,6 +43,8 @@ def parse():
     ap.add_argument("--options", type=lambda v: int(v, 0), default=0, help="nh_set_options bits (kernel variants)")
     ap.add_argument("--two-step", action="store_true", help="NH_OPT_LB_TWOSTEP: force two LB steps per launch through the L2")
     ap.add_argument("--one-step", action="store_true", help="NH_OPT_LB_ONESTEP: one LB step per launch")
+    ap.add_argument("--graph", action="store_true", help="NH_OPT_GRAPH: replay nh_step through CUDA graphs (pays where the LB "
+                    "launches are short and the two-step kernel does not apply, e.g. --config 5)")
     ap.add_argument("--block-order", action="store_true", help="NH_OPT_LB_BLOCKORDER: two-step units in blockIdx order")
     ap.add_argument("--leslie", type=float, default=0.0,
                     help="scale of the paper's Table-1 Leslie viscosities in the force (row f1; 0 = elastic stress only)")
@@ -308,6 +310,9 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --impl ours needs a CUDA device (there is no CPU path)")
     torch.cuda.set_device(local)
+    # a stream of its own: the lattice, the copies and the timing events all go to torch's current stream, and
+    # graph replay (--graph) cannot capture the legacy default stream
+    torch.cuda.set_stream(torch.cuda.Stream())
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if rank == 0:
@@ -328,7 +333,7 @@ def main():
     d_pinned = torch.from_numpy(d).pin_memory()
     lat.set_director(d_pinned)
     base_opt = (args.options | (nh.OPT_LB_TWOSTEP if args.two_step else 0) | (nh.OPT_LB_ONESTEP if args.one_step else 0)
-                | (nh.OPT_LB_BLOCKORDER if args.block_order else 0))
+                | (nh.OPT_LB_BLOCKORDER if args.block_order else 0) | (nh.OPT_GRAPH if args.graph else 0))
 
     def barrier():
         torch.cuda.synchronize()
@@ -359,7 +364,7 @@ def main():
     mlups = job_mlups(world, nf, r * args.steps, ms)
 
     # ---- second pass of the same K steps with a CUDA-event pair around every launch ---------------
-    lat.set_options(base_opt | nh.OPT_TIMING)
+    lat.set_options((base_opt & ~nh.OPT_GRAPH) | nh.OPT_TIMING)      # per-launch events need plain launches: same kernels
     barrier()
     for _ in range(args.steps):
         lat.step(r)
