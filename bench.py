@@ -384,7 +384,8 @@ def main():
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak,
                 "traffic": ncu_traffic(args.precision + ("+2step" if two else ""), desc["grid"]),
-                "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
+                "peak_source": peak_src, "frac_of_nominal_8000_gbs": achieved / 8000.0,
+                "algorithmic_bytes_per_launch": alg_bytes,
                 "lb_steps_per_launch": steps_per_launch,
                 "avg_launch_ms": lb_avg, "launches_timed": lb_n, "share_of_step": lb_ms / total_k if total_k else None,
                 "kernel_ms": {k: round(v[0], 4) for k, v in kt.items()},
