@@ -178,6 +178,9 @@ director_tile_kernel(const T* __restrict__ m, const T* __restrict__ u, const T* 
   unsigned c = (unsigned)z0 * G.plane + (unsigned)y * (unsigned)G.nx + (unsigned)x;
   const unsigned N = (unsigned)G.N;
   const T hdt = T(0.5) * C.dt;
+  // corrector: a = n + dt/2 k1 of the own cell, read one plane ahead so that its latency hides behind the stencil
+  V3<T> a_next = zero;
+  if (STAGE == 1 && active) a_next = {a_in[c], a_in[c + N], a_in[c + 2 * N]};
 
   for (int z = z0; z <= z1; ++z) {
     cp_async_wait_all();     // plane z+1 (enqueued one iteration ago)
@@ -188,6 +191,11 @@ director_tile_kernel(const T* __restrict__ m, const T* __restrict__ u, const T* 
       msrc += G.plane; usrc += G.plane;
     }
     cp_async_commit();
+    const V3<T> a_own = a_next;
+    if (STAGE == 1 && active && z < z1) {
+      const unsigned cn = c + G.plane;
+      a_next = {a_in[cn], a_in[cn + N], a_in[cn + 2 * N]};
+    }
     const T* pm = sm + sc * S::ELEMS;
     const V3<T> mzp = lds3<T, 1>(sm + sp * S::ELEMS, oc);
     V3<T> uzp = zero, dxu = zero, dyu = zero, dzu = zero;
@@ -208,8 +216,7 @@ director_tile_kernel(const T* __restrict__ m, const T* __restrict__ u, const T* 
         out_m[c] = v.x; out_m[c + N] = v.y; out_m[c + 2 * N] = v.z;
         a_out[c] = a.x; a_out[c + N] = a.y; a_out[c + 2 * N] = a.z;
       } else {
-        const V3<T> a = {a_in[c], a_in[c + N], a_in[c + 2 * N]};
-        const V3<T> v = unit_fast(a + hdt * k);
+        const V3<T> v = unit_fast(a_own + hdt * k);
         out_m[c] = v.x; out_m[c + N] = v.y; out_m[c + 2 * N] = v.z;
       }
     }
@@ -518,6 +525,12 @@ director3_tile_kernel(const T* __restrict__ m, const T* __restrict__ u, const T*
       src += G.plane; usrc += G.plane; ++zf;
     }
     cp_async_commit();
+    // corrector: a of the cell whose rate completes in this iteration, requested before the stencil work
+    V3<T> a_own = zero;
+    if (STAGE == 1 && active && p > z0) {
+      const unsigned cm = c - G.plane;
+      a_own = {a_in[cm], a_in[cm + N], a_in[cm + 2 * N]};
+    }
     T* sig = ssig + (p & 1) * SigShape::ELEMS;
     const T* pc = sn + (p & 3) * S::ELEMS;
     const T* pzm = sn + ((p - 1) & 3) * S::ELEMS;
@@ -574,8 +587,7 @@ director3_tile_kernel(const T* __restrict__ m, const T* __restrict__ u, const T*
           out_m[cm] = v.x; out_m[cm + N] = v.y; out_m[cm + 2 * N] = v.z;
           a_out[cm] = a.x; a_out[cm + N] = a.y; a_out[cm + 2 * N] = a.z;
         } else {
-          const V3<T> a = {a_in[cm], a_in[cm + N], a_in[cm + 2 * N]};
-          const V3<T> v = unit_fast(a + hdt * kk);
+          const V3<T> v = unit_fast(a_own + hdt * kk);
           out_m[cm] = v.x; out_m[cm + N] = v.y; out_m[cm + 2 * N] = v.z;
         }
       }
