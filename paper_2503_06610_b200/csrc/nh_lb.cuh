@@ -41,6 +41,10 @@ struct LbConst {
 template <typename T>
 struct Pop { T f[Q]; };
 
+// Programmatic dependent launch (PTX griddepcontrol; no-ops when the launch does not carry the attribute)
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ float fmaf_t(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ double fmaf_t(double a, double b, double c) { return fma(a, b, c); }
 
@@ -210,11 +214,16 @@ template <typename T, bool SHIFTED>
 __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 6 : 3)
 lb_step_kernel(const T* __restrict__ fsrc, T* __restrict__ fdst, const T* __restrict__ Flc,
                Geom G, LbConst<T> C, int reverse) {
+  // Programmatic dependent launch between consecutive LB steps (launch_lb sets the attribute only then): the next
+  // step's CTAs become resident as ours retire, and wait below before they read anything.  Every thread waits
+  // (also the ones that then leave), so that this grid cannot complete before its predecessor has.
+  grid_launch_dependents();
   const unsigned k = sweep_block(reverse) * blockDim.x + threadIdx.x;
-  if (k >= G.nfluid) return;
   int x, y, z;
-  cell_of(k, G, x, y, z);
+  cell_of(k < G.nfluid ? k : 0u, G, x, y, z);
   const size_t c = (size_t)k + G.plane;
+  grid_dependency_wait();
+  if (k >= G.nfluid) return;
   Pop<T> P;
   pull<T>(fsrc, G, x, y, z, P);
   T Fx = T(0), Fy = T(0), Fz = T(0);
