@@ -360,3 +360,45 @@ def test_two_lattices_interleaved_on_two_streams():
     fa, fb = ga.get_fields(), gb.get_fields()
     for k in ra:
         assert np.array_equal(fa[k], ra[k]) and np.array_equal(fb[k], rb[k]), k
+
+
+def test_chained_lb_launches_with_two_lattices_on_one_stream():
+    """Consecutive one-step LB launches are chained by programmatic dependent launch.  Two
+    lattices of different sizes stepped one LB step at a time in alternation on the SAME stream put the other
+    lattice's launch between every two of a lattice's own: each must still give exactly what it gives alone,
+    in plain launches and under graph replay."""
+    import torch
+    m = nh()
+    p = I.config(1, fd_ratio=7, nx=96, ny=40, nz=12)
+    d = p.pop("director")
+    p.pop("steps")
+    q = I.config(1, fd_ratio=3, nx=32, ny=24, nz=30, g=(-3e-7, 2e-7, 0.0), tau=0.9)
+    e = q.pop("director")
+    q.pop("steps")
+
+    def alone(par, n0):
+        g = m.Lattice(**dict(par, precision=1))
+        g.set_options(m.OPT_LB_ONESTEP)
+        g.set_director(n0)
+        g.step(60)
+        f = g.get_fields()
+        g.close()
+        return f
+
+    ra, rb = alone(p, d), alone(q, e)
+    for opt in (m.OPT_LB_ONESTEP, m.OPT_LB_ONESTEP | m.OPT_GRAPH):
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            ga = m.Lattice(stream=st, **dict(p, precision=1))
+            gb = m.Lattice(stream=st, **dict(q, precision=1))
+            for g, n0 in ((ga, d), (gb, e)):
+                g.set_options(opt)
+                g.set_director(n0)
+            for chunk in (1,) * 20 + (3, 2, 5, 10, 20):
+                ga.step(chunk)
+                gb.step(chunk)
+            fa, fb = ga.get_fields(), gb.get_fields()
+            ga.close()
+            gb.close()
+        for k in ra:
+            assert np.array_equal(fa[k], ra[k]) and np.array_equal(fb[k], rb[k]), (opt, k)
