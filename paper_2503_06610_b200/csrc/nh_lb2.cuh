@@ -203,6 +203,10 @@ __global__ void __launch_bounds__(NT, (sizeof(T) == 4 ? 4 : (U == 2 ? 1 : 2)) * 
 lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restrict__ Flc,
                Geom G, LbConst<T> C, Wave W) {
   const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  // programmatic dependent launch after another lb_wave launch (launch_lb2_u): resident early, but no ticket, no
+  // flag and no population is touched before the previous launch has completed
+  grid_launch_dependents();
+  grid_dependency_wait();
   // which unit: decoded once (by thread 0 from its ticket, or by everyone from blockIdx, which the
   // compiler keeps on the uniform datapath)
   int phase, k;
