@@ -127,8 +127,9 @@ long nh_launch_count(const nh_lattice* L);
  *   bit5 NH_OPT_FD_NOVEC      stage the FD tiles element by element even where 16-byte copies fit
  *   bit6 NH_OPT_LB_TWOSTEP    two LB steps per launch through an L2-resident plane ring wherever no
  *                             director update falls between them and the grid tiles into pieces
- *                             (nx a multiple of 64 that divides, or is a multiple of, 512; else one step
- *                             per launch);
+ *                             (nx a multiple of 64 that divides 512, is a multiple of 512, or has a
+ *                             factor 3, 5, 6 or 7 in nx / 64: 192, 320, 384, 448, 576, 640, ...; else
+ *                             one step per launch);
  *                             bit-identical results.  Without bit6 and bit7 the library decides
  *                             (FP32, planes >= 256x256, ring <= 48 MB: DESIGN.md section 7).
  *   bit7 NH_OPT_LB_ONESTEP    never use the two-step kernel

@@ -243,10 +243,22 @@ int launch_lb(nh_lattice* L) {
 // Geometry of one strip-plane for U cells per thread: YS lattice rows per strip (+ 2 halo rows in the
 // ring), cut into pieces of NT*U cells; false if this grid does not tile into pieces.
 struct PieceGrid { unsigned YS, nstrips, cps, ppr, rows_per_piece, pieces2; int spr_shift; };
-int lb2_threads(const nh_lattice* L) { return (L->options >> 31) & 1 ? 128 : 256; }
+// Threads per CTA for U cells per thread.  256 (or 128 when forced) where rows of nx cells tile into pieces of
+// 256 U cells; otherwise, for two cells per thread, 32 k threads with k the largest divisor of nx / 64 in 3..7
+// (one piece = k warps side by side in one row: nx = 320 -> 160 threads, 384 -> 192, 448 -> 224, 192 -> 96,
+// 576 -> 96 x 3 pieces per row); 0 if there is none.
+int lb2_threads(const nh_lattice* L, int U) {
+  if ((L->options >> 31) & 1) return 128;
+  const unsigned nx = (unsigned)L->G.nx, pc = 256u * U;
+  if (pc % nx == 0 || nx % pc == 0) return 256;
+  if (U != 2 || nx % 64) return 256;          // piece_grid will refuse
+  const unsigned n64 = nx / 64;
+  for (unsigned k = 7; k >= 3; --k) if (n64 % k == 0) return (int)(32 * k);
+  return 256;
+}
 bool piece_grid(const nh_lattice* L, int U, PieceGrid* g) {
-  const unsigned nx = (unsigned)L->G.nx, ny = (unsigned)L->G.ny, seg = 32u * U, pc = (unsigned)lb2_threads(L) * U;
-  const unsigned warps = (unsigned)lb2_threads(L) / 32;
+  const unsigned nx = (unsigned)L->G.nx, ny = (unsigned)L->G.ny, seg = 32u * U, pc = (unsigned)lb2_threads(L, U) * U;
+  const unsigned warps = (unsigned)lb2_threads(L, U) / 32;
   if (nx % seg) return false;
   // strips of about 64 K cells per plane (what was measured to pay), or 2^c of them when forced
   unsigned nstrips = 1;
@@ -268,7 +280,9 @@ bool piece_grid(const nh_lattice* L, int U, PieceGrid* g) {
   } else return false;
   g->spr_shift = 0;
   while ((1u << g->spr_shift) < spr) ++g->spr_shift;
-  return (1u << g->spr_shift) == spr;
+  // warp w of a piece works on segment w & (2^shift - 1) of row w >> shift: with one row per piece any number
+  // of warps up to 2^shift will do, with several rows per piece a row must hold a power of two of segments
+  return g->rows_per_piece == 1 || (1u << g->spr_shift) == spr;
 }
 int lb2_cells_per_thread(const nh_lattice* L) {
   PieceGrid g;
@@ -279,6 +293,12 @@ int lb2_cells_per_thread(const nh_lattice* L) {
 // Ring and lead of the wavefront (planes).  Defaults from the B200 measurements in DESIGN.md.
 void lb2_lead(const nh_lattice* L, const PieceGrid& g, int* D, int* R) {
   *D = (L->options >> 16) & 0xf; *R = (L->options >> 20) & 0x3f;
+  if (*D == 0 && *R == 0) {
+    // D = 4, R = 8 where eight ring planes stay within 48 MB of the L2; a shorter wavefront (D = 3, R = 6) for
+    // larger strip-planes (measured on 320x320x64: 35 600 against 34 800 MLUPS with the 63 MB ring, 32 600 one-step)
+    const double plane_mb = 19.0 * (g.YS + 2) * L->G.nx * word_of(L->p.precision) / 1e6;
+    if (8.0 * plane_mb > 48.0) { *D = 3; *R = 6; }
+  }
   if (*D == 0) *D = 4;
   if (*R == 0) *R = *D + 4;
   // the workspace holds ring_cap planes of (ny + 2) rows
@@ -389,8 +409,14 @@ int launch_lb2_u(nh_lattice* L) {
 template <typename T, bool SH>
 int launch_lb2(nh_lattice* L) {
   const bool two = lb2_cells_per_thread(L) == 2;
-  if (lb2_threads(L) == 128) return two ? launch_lb2_u<T, SH, 2, 128>(L) : launch_lb2_u<T, SH, 1, 128>(L);
-  return two ? launch_lb2_u<T, SH, 2, 256>(L) : launch_lb2_u<T, SH, 1, 256>(L);
+  switch (lb2_threads(L, two ? 2 : 1)) {
+    case 96: return launch_lb2_u<T, SH, 2, 96>(L);
+    case 160: return launch_lb2_u<T, SH, 2, 160>(L);
+    case 192: return launch_lb2_u<T, SH, 2, 192>(L);
+    case 224: return launch_lb2_u<T, SH, 2, 224>(L);
+    case 128: return two ? launch_lb2_u<T, SH, 2, 128>(L) : launch_lb2_u<T, SH, 1, 128>(L);
+    default: return two ? launch_lb2_u<T, SH, 2, 256>(L) : launch_lb2_u<T, SH, 1, 256>(L);
+  }
 }
 
 template <typename T, bool SH>

@@ -199,7 +199,7 @@ __device__ __forceinline__ void gather_cells(const Tab& S, unsigned zm, unsigned
 // its flags (the old readers of its ring slot) only before it stores; a phase-2 unit checks before
 // it gathers.  One barrier at the end, then thread 0 publishes the unit (fence, flag, counter).
 template <typename T, bool SHIFTED, int U, int NT>
-__global__ void __launch_bounds__(NT, (sizeof(T) == 4 ? 4 : (U == 2 ? 1 : 2)) * (256 / NT))
+__global__ void __launch_bounds__(NT, (sizeof(T) == 4 ? 1024 : (U == 2 ? 256 : 512)) / NT)
 lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restrict__ Flc,
                Geom G, LbConst<T> C, Wave W) {
   const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;

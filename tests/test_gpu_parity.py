@@ -230,7 +230,9 @@ def test_options_do_not_change_results():
 
 @pytest.mark.parametrize("shape,r", [((64, 64, 32), 10), ((128, 5, 20), 7), ((32, 7, 9), 3), ((512, 4, 6), 2),
                                      ((1024, 3, 5), 2), ((64, 3, 3), 2), ((256, 9, 8), 4), ((16, 16, 8), 1),
-                                     ((128, 24, 12), 3), ((512, 16, 9), 4), ((64, 40, 7), 2)])
+                                     ((128, 24, 12), 3), ((512, 16, 9), 4), ((64, 40, 7), 2),
+                                     # rows that do not tile into 512-cell pieces: CTAs of 160, 96, 224, 96 x 3, 160 x 2 threads
+                                     ((320, 6, 9), 3), ((192, 10, 8), 2), ((448, 4, 7), 4), ((576, 3, 6), 2), ((640, 4, 6), 3)])
 def test_two_step_kernel_is_bit_identical(shape, r):
     """The two-steps-per-sweep LB kernel (L2-resident plane ring, wavefront along z) does the same
     arithmetic per cell as the one-step kernel, so every field must agree bit for bit, whatever
