@@ -373,14 +373,17 @@ def main():
     # dominant kernel: the one-step LB launch, or the two-step launch (2 LB steps each) when it is on
     two = kt["lb2"][0] > kt["lb"][0]
     lb_ms, lb_n = kt["lb2"] if two else kt["lb"]
-    steps_per_launch = 2 if two else 1
+    # (small lattices take all the LB steps between two director updates in one cooperative launch)
+    steps_per_launch = 2 if two else max(1, int(round(r * args.steps / max(lb_n, 1))))
     lb_avg = lb_ms / max(lb_n, 1)
     total_k = sum(v[0] for v in kt.values())
     peak, peak_src = peaks()
     # 19 read + 19 write + 3 (F^LC) words per fluid cell and LB step
     alg_bytes = 41 * word * nf * steps_per_launch
     achieved = alg_bytes / (lb_avg * 1e-3) / 1e9 if lb_avg > 0 else 0.0
-    kname = "lb_wave (2 x collide+stream+force per launch)" if two else "lb_step (collide+stream+force)"
+    kname = ("lb_wave (2 x collide+stream+force per launch)" if two else
+             "lb_step (collide+stream+force)" if steps_per_launch == 1 else
+             "lb_resident (%d x collide+stream+force per cooperative launch, lattice resident in the L2)" % steps_per_launch)
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak,
                 "traffic": ncu_traffic(args.precision + ("+2step" if two else ""), desc["grid"]),

@@ -107,6 +107,7 @@ struct nh_lattice {
   unsigned order_len;
   int order_key;                   // (D << 8) | nzf the tables were built for, -1: none
   int sm_count;
+  int resident_blocks;             // co-resident CTAs of lb_resident_kernel on this device (-1: not asked yet)
   int chain_lb;                    // the last launch of this lattice: 1 lb_step_kernel, 2 lb_wave_kernel, 0 anything else
   int defer_force;                 // nh_defer_force: nh_step leaves F^LC to a later nh_update_force
   // CUDA-graph replay of nh_step (NH_OPT_GRAPH): one executable graph per distinct call shape
@@ -419,6 +420,39 @@ int launch_lb2(nh_lattice* L) {
   }
 }
 
+// ---- several LB steps in one cooperative launch (small lattices; lb_resident_kernel) -----------------
+// Usable when every fluid cell gets a thread of its own in one co-resident grid.  Not under graph replay (a
+// cooperative launch is kept out of captures) and not with NH_OPT_LB_ONESTEP (= one launch per LB step).
+template <typename T, bool SH>
+bool resident_usable(nh_lattice* L) {
+  if (L->options & (NH_OPT_LB_ONESTEP | NH_OPT_LB_TWOSTEP | NH_OPT_GRAPH | NH_OPT_LB_WIDE)) return false;
+  if (L->resident_blocks < 0) {
+    int per_sm = 0, coop = 0, dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, nh::lb_resident_kernel<T, SH>, BLOCK, 0) != cudaSuccess) {
+      cudaGetLastError();
+      coop = 0;
+    }
+    L->resident_blocks = coop ? per_sm * L->sm_count : 0;
+  }
+  return (long)blocks_for(L->G.nfluid) <= (long)L->resident_blocks;
+}
+template <typename T, bool SH>
+int launch_lb_resident(nh_lattice* L, int nsteps) {
+  Bracket br(L, KC_LB);
+  if (br.rc) return br.rc;
+  T* fa = (T*)L->f[L->cur];
+  T* fb = (T*)L->f[L->cur ^ 1];
+  const T* F = (const T*)L->F;
+  nh::Geom G = L->G;
+  nh::LbConst<T> C = lb_const<T>(L);
+  void* args[] = {&fa, &fb, &F, &G, &C, &nsteps};
+  NH_CUDA(cudaLaunchCooperativeKernel((const void*)nh::lb_resident_kernel<T, SH>, dim3(blocks_for(L->G.nfluid)), dim3(BLOCK),
+                                      args, 0, L->stream));
+  br.end();
+  return NH_OK;
+}
+
 template <typename T, bool SH>
 int launch_velocity(nh_lattice* L) {
   Bracket br(L, KC_VEL);
@@ -688,6 +722,16 @@ template <typename T, bool SH>
 int step_typed(nh_lattice* L, int n_lb, int r) {
   for (int s = 0; s < n_lb; ++s) {
     int rc;
+    // small lattice: all the steps up to the next director update (or the end of the call) in one launch
+    int m = n_lb - s;
+    if (r > 0 && m > r - (int)(L->t % r)) m = r - (int)(L->t % r);
+    if (m >= 16 && !lb2_usable(L) && resident_usable<T, SH>(L)) {   // (a cooperative launch costs about 10 us)
+      rc = launch_lb_resident<T, SH>(L, m);
+      if (rc) return rc;
+      L->t += m - 1;
+      s += m - 1;
+      if (!(m & 1)) L->cur ^= 1;       // (one more flip below)
+    } else
     // two steps in one launch when no director update falls between them
     if (s + 1 < n_lb && lb2_usable(L) && !(r > 0 && (L->t + 1) % r == 0)) {
       rc = launch_lb2<T, SH>(L);
@@ -968,7 +1012,7 @@ int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_strea
   L->ring_cap = ring_planes(p);
   L->ring = take((size_t)L->ring_cap * 19 * L->G.nx * (L->G.ny + 2) * w);
   L->wave = (unsigned long long*)take(wave_words(p) * 8);
-  L->wave_epoch = 0; L->wave_tickets = 0; L->order_key = -1;
+  L->wave_epoch = 0; L->wave_tickets = 0; L->order_key = -1; L->resident_blocks = -1;
   for (int i = 0; i < 32; ++i) L->strip_count[i] = 0;
   e = cudaMemsetAsync(L->wave, 0, wave_words(p) * 8, L->stream);
   if (e != cudaSuccess) { delete L; return cuda_fail(e, "cudaMemsetAsync(wave)"); }

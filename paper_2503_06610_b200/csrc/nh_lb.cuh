@@ -11,6 +11,7 @@
 // by one element along x.  Layout: SoA, f[i][z][y][x], x fastest.
 #pragma once
 #include <cuda_runtime.h>
+#include <cooperative_groups.h>
 
 namespace nh {
 
@@ -231,6 +232,38 @@ lb_step_kernel(const T* __restrict__ fsrc, T* __restrict__ fdst, const T* __rest
   collide<T, SHIFTED>(P, Fx, Fy, Fz, C);
 #pragma unroll
   for (int i = 0; i < Q; ++i) fdst[(size_t)i * G.N + c] = P.f[i];
+}
+
+// Small lattices (the whole grid resident on the SMs at once, the populations in the L2): `nsteps` LB steps in
+// ONE cooperative launch, a grid-wide barrier between steps, one thread per fluid cell for the whole launch.
+// Between two director updates the force is frozen, so it is read once.  Same gather and
+// collision as lb_step_kernel (bit-identical); the gathers go to the L2 (written by other CTAs one barrier ago).
+// Step s reads f[s & 1] and writes f[(s + 1) & 1].
+template <typename T, bool SHIFTED>
+__global__ void __launch_bounds__(256, sizeof(T) == 4 ? 4 : 2)
+lb_resident_kernel(T* __restrict__ fa, T* __restrict__ fb, const T* __restrict__ Flc, Geom G, LbConst<T> C, int nsteps) {
+  cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+  const unsigned k = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool on = k < G.nfluid;
+  int x, y, z;
+  cell_of(on ? k : 0u, G, x, y, z);
+  const size_t c = (size_t)(on ? k : 0u) + G.plane;
+  const PlaneMap M = lattice_map(G, z);
+  T Fx = T(0), Fy = T(0), Fz = T(0);
+  if (C.use_flc && on) { Fx = __ldg(Flc + c); Fy = __ldg(Flc + G.N + c); Fz = __ldg(Flc + 2 * G.N + c); }
+  T* src = fa;
+  T* dst = fb;
+  for (int s = 0; s < nsteps; ++s) {
+    if (on) {
+      Pop<T> P;
+      pull_map<T, LD_CG>(src, G, M, x, y, z == 1, z == G.nz - 2, P);
+      collide<T, SHIFTED>(P, Fx, Fy, Fz, C);
+#pragma unroll
+      for (int i = 0; i < Q; ++i) dst[(size_t)i * G.N + c] = P.f[i];
+    }
+    grid.sync();
+    T* t = src; src = dst; dst = t;
+  }
 }
 
 // rho, u of the populations that the NEXT step will gather (i.e. at the current time t), with the

@@ -404,3 +404,31 @@ def test_chained_lb_launches_with_two_lattices_on_one_stream():
             gb.close()
         for k in ra:
             assert np.array_equal(fa[k], ra[k]) and np.array_equal(fb[k], rb[k]), (opt, k)
+
+
+@pytest.mark.parametrize("shape,r", [((64, 64, 16), 20), ((16, 16, 8), 50), ((33, 7, 5), 16), ((64, 64, 32), 0)])
+def test_resident_multi_step_kernel_is_bit_identical(shape, r):
+    """Small lattices take all the LB steps between two director updates in ONE cooperative launch
+    (lb_resident_kernel, 16 steps or more): same arithmetic per cell as one launch per step, so bit for bit
+    the same fields, for uneven step() chunks; and far fewer launches."""
+    m = nh()
+    nx, ny, nz = shape
+    d = I.noisy_homeotropic(nx, ny, nz, 0.1)
+    p = dict(nx=nx, ny=ny, nz=nz, tau=0.7, K=0.004, pitch=9.0, xi=0.8, gamma1=1.3, g=(2e-6, -1e-6, 0.0), fd_ratio=r)
+    for precision in (0, 1, 2):
+        out = []
+        for opt, chunks in ((m.OPT_LB_ONESTEP, [137]), (0, [137]), (0, [1, 40, 17, 60, 19])):
+            g = m.Lattice(**dict(p, precision=precision))
+            g.set_options(opt)
+            g.set_director(d)
+            for c in chunks:
+                g.step(c)
+            out.append((g.get_fields(), g.launch_count))
+            assert g.time == 137
+            g.close()
+        for f, _ in out[1:]:
+            for k in out[0][0]:
+                assert np.array_equal(out[0][0][k], f[k]), (shape, precision, k)
+        # FP64 keeps 2 CTAs of 256 threads per SM resident (296 on 148 SMs): larger lattices stay on one launch per step
+        if precision != 0 or nx * ny * (nz - 2) <= 296 * 256:
+            assert out[1][1] < out[0][1] // 2
