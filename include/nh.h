@@ -132,7 +132,8 @@ long nh_launch_count(const nh_lattice* L);
  *                             one step per launch);
  *                             bit-identical results.  Without bit6 and bit7 the library decides
  *                             (FP32, planes >= 256x256, ring <= 48 MB: DESIGN.md section 7).
- *   bit7 NH_OPT_LB_ONESTEP    never use the two-step kernel
+ *   bit7 NH_OPT_LB_ONESTEP    one launch per LB step: neither the two-step kernel nor, on small lattices, the
+ *                             cooperative launch that takes all the steps up to the next director update
  *   bits 8-15                 planes per CTA of the tiled FD kernels (0 = chosen by the library)
  *   bits 16-19, 20-25         two-step kernel: lead D of phase 1 in planes, ring planes R (0 = default)
  *   bit26 NH_OPT_LB_BLOCKORDER two-step kernel: units in blockIdx order instead of by atomic ticket
