@@ -129,6 +129,7 @@ struct nh_lattice {
 namespace {
 
 constexpr int BLOCK = 256;
+constexpr int NH_EAGAIN = 1;   // internal: this way is not available here, take the plain one
 unsigned blocks_for(size_t n) { return (unsigned)((n + BLOCK - 1) / BLOCK); }
 
 int drain_events(nh_lattice* L) {
@@ -447,8 +448,16 @@ int launch_lb_resident(nh_lattice* L, int nsteps) {
   nh::Geom G = L->G;
   nh::LbConst<T> C = lb_const<T>(L);
   void* args[] = {&fa, &fb, &F, &G, &C, &nsteps};
-  NH_CUDA(cudaLaunchCooperativeKernel((const void*)nh::lb_resident_kernel<T, SH>, dim3(blocks_for(L->G.nfluid)), dim3(BLOCK),
-                                      args, 0, L->stream));
+  const cudaError_t e = cudaLaunchCooperativeKernel((const void*)nh::lb_resident_kernel<T, SH>, dim3(blocks_for(L->G.nfluid)),
+                                                    dim3(BLOCK), args, 0, L->stream);
+  if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorNotSupported) {
+    // fewer CTAs fit than the occupancy query promised (a shared device): one launch per step from now on
+    cudaGetLastError();
+    L->resident_blocks = 0;
+    L->launches -= 1; L->cnt[KC_LB] -= 1;
+    return NH_EAGAIN;
+  }
+  NH_CUDA(e);
   br.end();
   return NH_OK;
 }
@@ -725,9 +734,13 @@ int step_typed(nh_lattice* L, int n_lb, int r) {
     // small lattice: all the steps up to the next director update (or the end of the call) in one launch
     int m = n_lb - s;
     if (r > 0 && m > r - (int)(L->t % r)) m = r - (int)(L->t % r);
+    bool resident = false;
     if (m >= 16 && !lb2_usable(L) && resident_usable<T, SH>(L)) {   // (a cooperative launch costs about 10 us)
       rc = launch_lb_resident<T, SH>(L, m);
-      if (rc) return rc;
+      if (rc != NH_OK && rc != NH_EAGAIN) return rc;
+      resident = (rc == NH_OK);
+    }
+    if (resident) {
       L->t += m - 1;
       s += m - 1;
       if (!(m & 1)) L->cur ^= 1;       // (one more flip below)
@@ -842,7 +855,6 @@ int get_fields_typed(nh_lattice* L, double* rho, double* u, double* n, double* F
 
 int step_plain(nh_lattice* L, int n_lb, int r);
 int step_graph(nh_lattice* L, int n_lb, int r);
-constexpr int NH_EAGAIN = 1;   // internal: fall back to plain launches
 
 #define NH_DISPATCH(L, CALL_F64S, CALL_F32S, CALL_F32U, CALL_F64U) \
   switch ((L)->p.precision) {                                      \
