@@ -159,6 +159,35 @@ def test_P13_advected_shear_wave(axis):
     assert abs(amp / (A * math.exp(-nu * k * k * T)) - 1.0) < 0.01
 
 
+@pytest.mark.parametrize("gz", [1e-4, -1e-4])
+@pytest.mark.parametrize("tau", [0.8, 1.0])
+def test_P14_hydrostatic_column_pins_the_z_orientation_of_streaming(gz, tau):
+    """P14: LC coupling off, body acceleration along z only.  With u = 0 Eq. 1 reduces
+    to c_s^2 d(rho)/dz = rho g_z with c_s^2 = 1/3: ln rho rises by 3 g_z per layer
+    TOWARD +z for g_z > 0.  Populations move to x + e_i (Eq. 14 / Eq. 23 LHS)
+    and are reflected at the plate between two nodes; a stream mirrored in z stacks
+    the fluid on the other plate.  None of P1, P2, P3 (mirror-symmetric in z), P12 (uniform state)
+    or P13 (x and y) would notice that.  Expected values are from the hydrostatic balance, with the
+    O(g_z^2) lattice correction as the tolerance."""
+    nz = 14
+    o = Oracle(3, 2, nz, tau=tau, K=0.0, g=(0.0, 0.0, gz), fd_ratio=0, precision=0, coupling=0)
+    # transient: after a few steps mass has moved along the acceleration, away from one plate, onto the other
+    o.step(3, 0)
+    rho = o.get_fields()["rho"][:, 0, 0]
+    far, near = (nz - 2, 1) if gz > 0 else (1, nz - 2)
+    assert rho[far] > 1.0 + abs(gz) and rho[near] < 1.0 - abs(gz)
+    # steady state (acoustic modes damp with nu k^2; (nz-2)^2/nu ~ 1.4e3 steps, run 30x that)
+    o.step(40000, 0)
+    f = o.get_fields()
+    rho = f["rho"][1:-1]
+    assert np.abs(f["u"]).max() <= gz * gz  # at rest up to the O(g^2) lattice term (measured 0.25 g^2)
+    dln = np.diff(np.log(rho[:, 0, 0]))
+    assert np.all(dln * np.sign(gz) > 0.0)  # denser toward +z for g_z > 0, toward -z for g_z < 0
+    assert np.abs(dln / (3.0 * gz) - 1.0).max() < 2.0 * gz * gz  # measured 0.75 g^2
+    assert np.abs(rho - rho[:, :1, :1]).max() == 0.0  # uniform in x and y
+    assert abs((rho - 1.0).sum()) < 1e-12 * rho.size  # mass (P2) under a wall-normal force
+
+
 # ------------------------------------------------------------------------------------------
 # FD side
 # ------------------------------------------------------------------------------------------
