@@ -58,6 +58,7 @@ def parse():
                          "held by one process (measures the decomposition's overhead)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the sustained (>= 3 s) loop and the fp64 / one_step sub-records")
     return ap.parse_args()
 
 
@@ -103,22 +104,46 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic(precision_name, grid, with_inst=False):
-    """DRAM bytes per LB launch from the committed ncu --set full capture (profiles/lb_traffic.csv), or None."""
+LB_SOURCES = ("paper_2503_06610_b200/csrc/nh_lb.cuh", "paper_2503_06610_b200/csrc/nh_lb2.cuh")
+
+
+def lb_source_sha():
+    """First 16 hex digits of the SHA-256 of the LB kernel sources: profiles/lb_traffic.csv records the value a
+    capture was taken at, so that a capture of an older kernel is never quoted for a newer one."""
+    import hashlib
+    h = hashlib.sha256()
+    for rel in LB_SOURCES:
+        with open(os.path.join(ROOT, rel), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(precision_name, grid):
+    """(DRAM bytes per launch, warp instructions per launch, where it comes from) of the dominant LB kernel, from
+    the committed `ncu --set full` capture (profiles/lb_traffic.csv: a STORED capture, not measured in this run).
+    Only a row taken from the kernel source as it stands now counts: otherwise (None, None, why)."""
     path = os.path.join(ROOT, "profiles", "lb_traffic.csv")
     if not os.path.exists(path):
-        return (None, None) if with_inst else None
+        return None, None, "no capture (profiles/lb_traffic.csv missing)"
     try:
         want = "%dx%dx%d" % tuple(grid)
-        val = inst = None
+        now = lb_source_sha()
+        row = stale = None
         for line in open(path).read().splitlines()[1:]:
             c = line.split(",")
-            if len(c) >= 4 and c[0] == precision_name and c[1] == want:
-                val = float(c[3])     # the last matching row is the newest capture
-                inst = float(c[5]) if len(c) >= 6 and c[5] else None
-        return (val, inst) if with_inst else val
-    except Exception:
-        return (None, None) if with_inst else None
+            if len(c) >= 5 and c[0] == precision_name and c[1] == want:
+                if len(c) >= 7 and c[6] == now:
+                    row = c                  # the last matching row is the newest capture
+                else:
+                    stale = c
+        if row is not None:
+            return float(row[3]), (float(row[5]) if row[5] else None), "stored capture %s (kernel source sha %s)" % (row[4], now)
+        if stale is not None:
+            return None, None, ("stale: the newest capture of this kernel and grid (%s) was taken from another version "
+                                "of the kernel source (now %s)" % (stale[4], now))
+        return None, None, "no capture for %s on %s" % (precision_name, want)
+    except Exception as e:  # noqa: BLE001
+        return None, None, "unreadable capture table: %s" % e
 
 
 class ClockSampler:
@@ -334,6 +359,8 @@ def main():
     lat.set_director(d_pinned)
     base_opt = (args.options | (nh.OPT_LB_TWOSTEP if args.two_step else 0) | (nh.OPT_LB_ONESTEP if args.one_step else 0)
                 | (nh.OPT_LB_BLOCKORDER if args.block_order else 0) | (nh.OPT_GRAPH if args.graph else 0))
+    l2_bytes = int(getattr(torch.cuda.get_device_properties(local), "L2_cache_size", 0)) or 126 * 1024 * 1024
+    peak, peak_src = peaks()
 
     def barrier():
         torch.cuda.synchronize()
@@ -350,65 +377,112 @@ def main():
         barrier()
         return max_over_ranks(ev0.elapsed_time(ev1), world)
 
-    # ---- device-resident timing: W warm-up steps, then exactly K steps ----------------------------
-    lat.set_options(base_opt)
-    for _ in range(args.warmup):
-        lat.step(r)
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    l0 = lat.launch_count
-    ms = timed(lambda: [lat.step(r) for _ in range(args.steps)])
-    launches = lat.launch_count - l0
-    clocks = sampler.stop() if rank == 0 else None
-    mlups = job_mlups(world, nf, r * args.steps, ms)
-
-    # ---- second pass of the same K steps with a CUDA-event pair around every launch ---------------
-    lat.set_options((base_opt & ~nh.OPT_GRAPH) | nh.OPT_TIMING)      # per-launch events need plain launches: same kernels
-    barrier()
-    for _ in range(args.steps):
-        lat.step(r)
-    kt = {k: lat.kernel_time(k) for k in nh.KERNEL_CLASSES}
-    lat.set_options(base_opt)
-    # dominant kernel: the one-step LB launch, or the two-step launch (2 LB steps each) when it is on
-    two = kt["lb2"][0] > kt["lb"][0]
-    lb_ms, lb_n = kt["lb2"] if two else kt["lb"]
-    # (small lattices take all the LB steps between two director updates in one cooperative launch)
-    steps_per_launch = 2 if two else max(1, int(round(r * args.steps / max(lb_n, 1))))
-    lb_avg = lb_ms / max(lb_n, 1)
-    total_k = sum(v[0] for v in kt.values())
-    peak, peak_src = peaks()
-    # 19 read + 19 write + 3 (F^LC) words per fluid cell and LB step
-    alg_bytes = 41 * word * nf * steps_per_launch
-    achieved = alg_bytes / (lb_avg * 1e-3) / 1e9 if lb_avg > 0 else 0.0
-    kname = ("lb_wave (2 x collide+stream+force per launch)" if two else
-             "lb_step (collide+stream+force)" if steps_per_launch == 1 else
-             "lb_resident (%d x collide+stream+force per cooperative launch, lattice resident in the L2)" % steps_per_launch)
-    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak,
-                "traffic": ncu_traffic(args.precision + ("+2step" if two else ""), desc["grid"]),
+    def measure(L, opt, precision_name, w, steps, warmup, sample_clocks=True):
+        """W warm-up steps, exactly K steps between barriers (CUDA events, max over ranks), then a second pass of the
+        same K steps with a CUDA-event pair around every launch for the dominant kernel's roofline."""
+        L.set_options(opt)
+        for _ in range(warmup):
+            L.step(r)
+        sampler = ClockSampler(local)
+        if rank == 0 and sample_clocks:
+            sampler.start()
+        l0 = L.launch_count
+        ms = timed(lambda: [L.step(r) for _ in range(steps)])
+        launches = L.launch_count - l0
+        clocks = sampler.stop() if rank == 0 and sample_clocks else None
+        L.set_options((opt & ~nh.OPT_GRAPH) | nh.OPT_TIMING)      # per-launch events need plain launches: same kernels
+        barrier()
+        for _ in range(steps):
+            L.step(r)
+        kt = {k: L.kernel_time(k) for k in nh.KERNEL_CLASSES}
+        L.set_options(opt)
+        # dominant kernel: the one-step LB launch, or the two-step launch (2 LB steps each) when it is on
+        two = kt["lb2"][0] > kt["lb"][0]
+        lb_ms, lb_n = kt["lb2"] if two else kt["lb"]
+        # (small lattices take all the LB steps between two director updates in one cooperative launch)
+        steps_per_launch = 2 if two else max(1, int(round(r * steps / max(lb_n, 1))))
+        lb_avg = lb_ms / max(lb_n, 1)
+        total_k = sum(v[0] for v in kt.values())
+        # 19 read + 19 write + 3 (F^LC) words per fluid cell and LB step (DESIGN.md section 5)
+        alg_bytes = 41 * w * nf * steps_per_launch
+        achieved = alg_bytes / (lb_avg * 1e-3) / 1e9 if lb_avg > 0 else 0.0
+        kname = ("lb_wave (2 x collide+stream+force per launch)" if two else
+                 "lb_step (collide+stream+force)" if steps_per_launch == 1 else
+                 "lb_resident (%d x collide+stream+force per cooperative launch)" % steps_per_launch)
+        traffic, inst, tsrc = ncu_traffic(precision_name + ("+2step" if two else ""), desc["grid"])
+        pop_bytes = 2 * 19 * N * w
+        in_l2 = pop_bytes <= l2_bytes
+        roof = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": tsrc,
                 "peak_source": peak_src, "frac_of_nominal_8000_gbs": achieved / 8000.0,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "lb_steps_per_launch": steps_per_launch,
                 "avg_launch_ms": lb_avg, "launches_timed": lb_n, "share_of_step": lb_ms / total_k if total_k else None,
                 "kernel_ms": {k: round(v[0], 4) for k, v in kt.items()},
-                "full_step_bytes_per_cell": (41 + 30.0 / r) * word,
-                "full_step_achieved_gbs": (41 + 30.0 / r) * word * nf * r * args.steps / (ms * 1e-3) / 1e9,
+                "full_step_bytes_per_cell": (41 + 30.0 / r) * w,
+                "full_step_achieved_gbs": (41 + 30.0 / r) * w * nf * r * steps / (ms * 1e-3) / 1e9,
                 "timed": "second pass of the same K steps with per-launch CUDA events on the launch stream"}
-    if roofline["traffic"] and lb_avg > 0:
-        # what the DRAM actually moved (ncu capture of the same kernel) over the live launch time
-        roofline["dram_gbs"] = roofline["traffic"] / (lb_avg * 1e-3) / 1e9
-        roofline["dram_frac"] = roofline["dram_gbs"] / peak
-    inst = ncu_traffic(args.precision + ("+2step" if two else ""), desc["grid"], with_inst=True)[1]
-    if inst and lb_avg > 0 and clocks and clocks.get("sm_mhz"):
-        # second ceiling: warp instructions issued against 148 SMs x 4 issue slots per clock
-        issue_peak = 148 * 4 * clocks["sm_mhz"] * 1e6
-        roofline["issue_frac"] = inst / (lb_avg * 1e-3) / issue_peak
-        roofline["warp_instructions_per_launch"] = inst
-    if two:
-        roofline["note"] = ("two LB steps share one pass over HBM (the intermediate step lives in an L2-resident "
+        if in_l2:
+            roof["resident_in_l2"] = True
+            roof["note"] = ("both population buffers (%.1f MB) fit the %.0f MB L2: the gathers are served by the L2, "
+                            "`achieved` is algorithmic bytes over time and says nothing about HBM; SURVEY 8(d): report "
+                            "MLUPS for such grids, not GB/s" % (pop_bytes / 1e6, l2_bytes / 1e6))
+        if traffic and lb_avg > 0:
+            # what the DRAM moved in the STORED ncu capture of this same kernel source, over the live launch time
+            roof["dram_gbs"] = traffic / (lb_avg * 1e-3) / 1e9
+            roof["dram_frac"] = roof["dram_gbs"] / peak
+            roof["dram_gbs_is"] = "derived: stored capture's bytes / this run's launch time"
+        if inst and lb_avg > 0 and clocks and clocks.get("sm_mhz"):
+            # second ceiling: warp instructions issued against SMs x 4 issue slots per clock (DESIGN.md section 5)
+            sms = torch.cuda.get_device_properties(local).multi_processor_count
+            roof["issue_frac"] = inst / (lb_avg * 1e-3) / (sms * 4 * clocks["sm_mhz"] * 1e6)
+            roof["warp_instructions_per_launch"] = inst
+        if two:
+            roof["note"] = ("two LB steps share one pass over HBM (the intermediate step lives in an L2-resident "
                             "plane ring), so the algorithmic bytes of two steps move in about the DRAM traffic of "
                             "one: frac > 1 is expected; dram_frac is the DRAM's own utilisation")
+        return {"ms": ms, "mlups": job_mlups(world, nf, r * steps, ms), "launches": launches, "clocks": clocks,
+                "roofline": roof, "pop_bytes": pop_bytes, "in_l2": in_l2}
+
+    # ---- the headline: device-resident timing, W warm-up steps, then exactly K steps ---------------
+    m = measure(lat, base_opt, args.precision, word, args.steps, args.warmup)
+    ms, mlups, launches, clocks, roofline = m["ms"], m["mlups"], m["launches"], m["clocks"], m["roofline"]
+
+    # ---- the same loop kept up for >= 3 s: does the number hold once power management has had time to act? ----
+    sustained = None
+    if not args.no_extras:
+        reps = max(args.steps, int(3000.0 / max(ms / args.steps, 1e-3)) + 1)
+        sampler = ClockSampler(local)
+        if rank == 0:
+            sampler.start()
+        ms_long = timed(lambda: [lat.step(r) for _ in range(reps)])
+        cl = sampler.stop() if rank == 0 else None
+        sustained = {"value": job_mlups(world, nf, r * reps, ms_long), "unit": "MLUPS", "steps": reps,
+                     "seconds": ms_long * 1e-3, "ms_per_step": ms_long / reps, "clocks": cl,
+                     "what": "the headline loop (same lattice, same options) repeated back to back for at least 3 s, "
+                             "clocks and throttle reasons sampled over that window"}
+
+    # ---- what `metric` also names: FP64, and the one-step FP32 kernel, each timed like the headline ----
+    extras = {}
+    if not args.no_extras and world == 1:
+        def sub(precision_name, opt):
+            pr = PRECISIONS[precision_name]
+            w2 = 8 if pr in (0, 3) else 4
+            L2 = nh.Lattice(device="cuda:%d" % local, **dict(p, precision=pr))
+            L2.set_director(d_pinned)
+            mm = measure(L2, opt, precision_name, w2, args.steps, args.warmup)
+            L2.close()
+            rf = mm["roofline"]
+            return {"value": mm["mlups"], "unit": "MLUPS", "ms_per_step": mm["ms"] / args.steps, "dtype": DTYPE[pr],
+                    "options": opt, "gpu_launches": mm["launches"], "clocks": mm["clocks"],
+                    "roofline": {k: rf.get(k) for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic",
+                                                        "traffic_source", "avg_launch_ms", "launches_timed",
+                                                        "share_of_step", "lb_steps_per_launch", "kernel_ms",
+                                                        "full_step_achieved_gbs", "resident_in_l2")}}
+        if args.precision != "fp64":
+            extras["fp64"] = sub("fp64", base_opt)
+        if not (base_opt & nh.OPT_LB_ONESTEP) and roofline["lb_steps_per_launch"] != 1:
+            extras["one_step"] = sub(args.precision, (base_opt & ~nh.OPT_LB_TWOSTEP) | nh.OPT_LB_ONESTEP)
 
     # ---- end to end through the C ABI with host buffers --------------------------------------------
     e2e = None
@@ -449,9 +523,16 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": DTYPE[prec], "data": "synthetic",
             "config": dict(desc, lb_steps_per_step=r, fluid_cells=nf, parallelism="replicas x%d" % world,
-                           l2="populations (2 x %.0f MB) exceed the 126 MB L2; no flush needed" % (19 * N * word / 1e6),
+                           l2=(("populations (2 x %.0f MB) exceed the %.0f MB L2; no flush needed"
+                                if not m["in_l2"] else
+                                "populations (2 x %.1f MB) FIT the %.0f MB L2 and nothing is flushed between steps: this grid is "
+                                "L2-resident by nature (a time step follows a time step); MLUPS is the figure, GB/s is not")
+                               % (19 * N * word / 1e6, l2_bytes / 1e6)),
                            options=base_opt),
             "clocks": clocks, "gpu_launches": launches, "roofline": roofline}
+    if sustained is not None:
+        line["sustained"] = sustained
+    line.update(extras)
     if e2e is not None:
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:
