@@ -45,7 +45,8 @@ def parse():
     ap.add_argument("--one-step", action="store_true", help="NH_OPT_LB_ONESTEP: one LB step per launch")
     ap.add_argument("--graph", action="store_true", help="NH_OPT_GRAPH: replay nh_step through CUDA graphs (pays where the LB "
                     "launches are short and the two-step kernel does not apply, e.g. --config 5)")
-    ap.add_argument("--block-order", action="store_true", help="NH_OPT_LB_BLOCKORDER: two-step units in blockIdx order")
+    ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
+                    help="nh_debug_tune knob (include/nh_debug.h), e.g. --tune lb2_lead=3 --tune lb2_ring=6")
     ap.add_argument("--leslie", type=float, default=0.0,
                     help="scale of the paper's Table-1 Leslie viscosities in the force (row f1; 0 = elastic stress only)")
     ap.add_argument("--fd-ratio", type=int, default=None, help="override the config's Delta t_FD / Delta t_LB")
@@ -358,7 +359,9 @@ def main():
     d_pinned = torch.from_numpy(d).pin_memory()
     lat.set_director(d_pinned)
     base_opt = (args.options | (nh.OPT_LB_TWOSTEP if args.two_step else 0) | (nh.OPT_LB_ONESTEP if args.one_step else 0)
-                | (nh.OPT_LB_BLOCKORDER if args.block_order else 0) | (nh.OPT_GRAPH if args.graph else 0))
+                | (nh.OPT_GRAPH if args.graph else 0))
+    knobs = {kv.split("=")[0]: int(kv.split("=")[1]) for kv in args.tune}
+    lat.debug_tune(**knobs)
     l2_bytes = int(getattr(torch.cuda.get_device_properties(local), "L2_cache_size", 0)) or 126 * 1024 * 1024
     peak, peak_src = peaks()
 
@@ -469,6 +472,7 @@ def main():
             pr = PRECISIONS[precision_name]
             w2 = 8 if pr in (0, 3) else 4
             L2 = nh.Lattice(device="cuda:%d" % local, **dict(p, precision=pr))
+            L2.debug_tune(**knobs)
             L2.set_director(d_pinned)
             mm = measure(L2, opt, precision_name, w2, args.steps, args.warmup)
             L2.close()
@@ -528,7 +532,7 @@ def main():
                                 "populations (2 x %.1f MB) FIT the %.0f MB L2 and nothing is flushed between steps: this grid is "
                                 "L2-resident by nature (a time step follows a time step); MLUPS is the figure, GB/s is not")
                                % (19 * N * word / 1e6, l2_bytes / 1e6)),
-                           options=base_opt),
+                           options=base_opt, tune=knobs),
             "clocks": clocks, "gpu_launches": launches, "roofline": roofline}
     if sustained is not None:
         line["sustained"] = sustained

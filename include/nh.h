@@ -31,6 +31,10 @@
  *     alive until nh_free.  The library owns only the handle.
  *   - All device work is enqueued on the stream given to nh_init_lattice.  nh_set_director and
  *     nh_get_fields synchronise that stream before returning; nh_step does not.
+ *   - Errors that happen ON the device after an asynchronous call has returned (a wavefront dependency of the
+ *     two-step LB kernel that is not met within its time bound, which would mean the launch order it relies on
+ *     was violated) are sticky: the kernel records them in host-visible memory, the launch ends, and every later
+ *     call that touches the lattice -- nh_step included -- returns NH_ECUDA; the lattice's state is then invalid.
  */
 #ifndef NH_H
 #define NH_H
@@ -115,41 +119,31 @@ long nh_time(const nh_lattice* L);
 long nh_launch_count(const nh_lattice* L);
 
 /* Options (results agree within round-off whatever they are):
- *   bit0 NH_OPT_GRAPH         replay nh_step through CUDA graphs (launch-bound small grids): one
- *                             executable graph per distinct (n_lb, r, t mod r, buffer parity), captured
- *                             on first use.  Needs a capturable stream (not the legacy default
- *                             stream), otherwise plain launches; excludes NH_OPT_LB_TWOSTEP.
- *   bit1 NH_OPT_TIMING        bracket every kernel launch with a CUDA-event pair on the lattice's
- *                             stream (ignored while graphs are on)
- *   bit2 NH_OPT_FD_DIRECT     use the one-thread-per-cell FD kernels instead of the tiled ones
- *   bit3 NH_OPT_LB_WIDE       use the 16-byte-per-thread LB kernel (needs nx % 4 == 0 in FP32, % 2 in FP64)
- *   bit4 NH_OPT_NO_SERPENTINE sweep the populations in the same direction on every launch
- *   bit5 NH_OPT_FD_NOVEC      stage the FD tiles element by element even where 16-byte copies fit
- *   bit6 NH_OPT_LB_TWOSTEP    two LB steps per launch through an L2-resident plane ring wherever no
- *                             director update falls between them and the grid tiles into pieces
- *                             (nx a multiple of 64 that divides 512, is a multiple of 512, or has a
- *                             factor 3, 5, 6 or 7 in nx / 64: 192, 320, 384, 448, 576, 640, ...; else
- *                             one step per launch);
- *                             bit-identical results.  Without bit6 and bit7 the library decides
- *                             (FP32, planes >= 256x256, ring <= 48 MB: DESIGN.md section 7).
- *   bit7 NH_OPT_LB_ONESTEP    one launch per LB step: neither the two-step kernel nor, on small lattices, the
- *                             cooperative launch that takes all the steps up to the next director update
- *   bits 8-15                 planes per CTA of the tiled FD kernels (0 = chosen by the library)
- *   bits 16-19, 20-25         two-step kernel: lead D of phase 1 in planes, ring planes R (0 = default)
- *   bit26 NH_OPT_LB_BLOCKORDER two-step kernel: units in blockIdx order instead of by atomic ticket
- *   bits 27-29                two-step kernel: log2 of the number of y-strips (0 = chosen by the library:
- *                             strips of about 64 K cells per plane; ny must be divisible by it)
- *   bits 30, 31               two-step kernel: one cell per thread; 128-thread CTAs (tuning)
+ *   NH_OPT_GRAPH         replay nh_step through CUDA graphs (launch-bound small grids): one executable graph per
+ *                        distinct (n_lb, r, t mod r, buffer parity), captured on first use.  Needs a capturable
+ *                        stream (not the legacy default stream), otherwise plain launches; the two-step LB kernel
+ *                        and the small-lattice cooperative launch are not used under it.
+ *   NH_OPT_TIMING        bracket every kernel launch with a CUDA-event pair on the lattice's stream (ignored while
+ *                        graphs are on)
+ *   NH_OPT_FD_DIRECT     use the one-thread-per-cell FD kernels instead of the tiled ones (cross-check form)
+ *   NH_OPT_NO_SERPENTINE sweep the populations in the same direction on every launch
+ *   NH_OPT_FD_NOVEC      stage the FD tiles element by element even where 16-byte copies fit
+ *   NH_OPT_LB_TWOSTEP    two LB steps per launch through an L2-resident plane ring wherever no director update
+ *                        falls between them and the grid tiles into pieces (nx a multiple of 64 that divides 512,
+ *                        is a multiple of 512, or has a factor 3, 5, 6 or 7 in nx / 64; else one step per launch);
+ *                        bit-identical results.  With neither this nor NH_OPT_LB_ONESTEP the library decides (FP32,
+ *                        planes >= 256x256, ring <= 48 MB: DESIGN.md section 7).
+ *   NH_OPT_LB_ONESTEP    one launch per LB step: neither the two-step kernel nor, on small lattices, the
+ *                        cooperative launch that takes all the steps up to the next director update
+ * Launch-shape tuning knobs are not part of this contract (include/nh_debug.h).
  * Setting options resets the timing accumulators. */
 #define NH_OPT_GRAPH          1
 #define NH_OPT_TIMING         2
 #define NH_OPT_FD_DIRECT      4
-#define NH_OPT_LB_WIDE        8
 #define NH_OPT_NO_SERPENTINE 16
 #define NH_OPT_FD_NOVEC      32
 #define NH_OPT_LB_TWOSTEP    64
 #define NH_OPT_LB_ONESTEP   128
-#define NH_OPT_LB_BLOCKORDER (1 << 26)
 int nh_set_options(nh_lattice* L, int options);
 
 /* Accumulated CUDA-event time (ms) and number of launches of one kernel class since the last

@@ -15,13 +15,15 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libnh_b200.so")
 
 FP64_SHIFTED, FP32_SHIFTED, FP32_UNSHIFTED, FP64_UNSHIFTED = 0, 1, 2, 3
-OPT_GRAPH, OPT_TIMING, OPT_FD_DIRECT, OPT_LB_WIDE, OPT_NO_SERPENTINE, OPT_FD_NOVEC, OPT_LB_TWOSTEP = 1, 2, 4, 8, 16, 32, 64
-OPT_LB_ONESTEP, OPT_LB_BLOCKORDER = 128, 1 << 26
+OPT_GRAPH, OPT_TIMING, OPT_FD_DIRECT, OPT_NO_SERPENTINE, OPT_FD_NOVEC, OPT_LB_TWOSTEP, OPT_LB_ONESTEP = 1, 2, 4, 16, 32, 64, 128
+# keys of nh_debug_tune (include/nh_debug.h: tuning and test hooks, not part of the contract)
+TUNE = {"fd_planes": 0, "lb2_lead": 1, "lb2_ring": 2, "lb2_strips": 3, "lb2_cells": 4, "lb2_threads": 5,
+        "lb2_blockorder": 6, "lb2_timeout_ms": 7, "lb2_fault": 8}
 KERNEL_CLASSES = ("lb", "velocity", "predictor", "corrector", "force", "other", "lb2")
 
 EXPORTS = ("nh_workspace_bytes", "nh_init_lattice", "nh_set_director", "nh_step", "nh_get_fields",
            "nh_time", "nh_launch_count", "nh_set_options", "nh_kernel_time", "nh_free", "nh_last_error",
-           "nh_rows_bytes", "nh_get_rows", "nh_set_rows", "nh_update_force", "nh_defer_force")
+           "nh_rows_bytes", "nh_get_rows", "nh_set_rows", "nh_update_force", "nh_defer_force", "nh_debug_tune")
 
 
 class NhParams(C.Structure):
@@ -73,6 +75,7 @@ def load():
         lib.nh_set_rows.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
         lib.nh_update_force.argtypes = [C.c_void_p]
         lib.nh_defer_force.argtypes = [C.c_void_p, C.c_int]
+        lib.nh_debug_tune.argtypes = [C.c_void_p, C.c_int, C.c_int]
         lib.nh_free.argtypes = [C.c_void_p]
         lib.nh_free.restype = None
         lib.nh_last_error.restype = C.c_char_p
@@ -167,6 +170,11 @@ class Lattice:
 
     def set_options(self, options):
         _check(load().nh_set_options(self._h, int(options)))
+
+    def debug_tune(self, **knobs):
+        """nh_debug_tune for each name=value (names: binding.TUNE); 0 = the library decides."""
+        for name, value in knobs.items():
+            _check(load().nh_debug_tune(self._h, TUNE[name], int(value)))
 
     def kernel_time(self, which):
         """(total ms, launches) of a kernel class since the last set_options (needs OPT_TIMING)."""

@@ -3,6 +3,7 @@
 // timing per kernel class.  No arithmetic of the method lives here: every step runs in the
 // kernels of nh_lb.cuh / nh_fd.cuh.
 #include "../../include/nh.h"
+#include "../../include/nh_debug.h"
 
 #include <cuda_runtime.h>
 
@@ -18,7 +19,6 @@
 #include "nh_frank3.cuh"
 #include "nh_lb.cuh"
 #include "nh_lb2.cuh"
-#include "nh_lb_vec.cuh"
 
 namespace {
 
@@ -67,10 +67,11 @@ enum KernelClass { KC_LB = 0, KC_VEL = 1, KC_PRED = 2, KC_CORR = 3, KC_FORCE = 4
 
 // planes of the two-step kernel's ring (nh_lb2.cuh) that the workspace holds
 int ring_planes(const nh_params* p) { return p->nz - 2 < 12 ? p->nz - 2 : 12; }
-// u64 words of the two-step kernel's control block: 8 header words, then two u32 flags per plane and piece
+// u64 words of the two-step kernel's control block: 8 header words, 32 strip counters, two u64 flags per plane and
+// piece, the order table (two u32 per plane, rounded up)
 size_t wave_words(const nh_params* p) {
   const size_t pieces = (size_t)p->nx * (p->ny + 2) / 128 + p->ny + 3;   // = lb2_max_pieces: bound over the piece shapes
-  return 8 + 32 + (size_t)(p->nz - 2) * pieces + (size_t)(p->nz - 2) + 8;   // header, strip counters, flags, order table
+  return 8 + 32 + 2 * (size_t)(p->nz - 2) * pieces + (size_t)(p->nz - 2) + 8;
 }
 
 }  // namespace
@@ -83,6 +84,7 @@ struct nh_lattice {
   long t;
   long launches;
   int options;
+  int tune[NH_TUNE_COUNT];   // nh_debug_tune: 0 = the library decides
   // device pointers into the caller's workspace (type-erased; word = 4 or 8 bytes)
   void* f[2];       // population ping-pong; f[cur] is what the next LB step gathers from
   int cur;
@@ -100,12 +102,14 @@ struct nh_lattice {
   int sweep;        // direction of the next population sweep (alternates, see sweep_block)
   void* ring;       // plane ring of the two-step LB kernel
   int ring_cap;     // planes it holds
-  unsigned long long* wave;   // device counters of the two-step kernel: err flag at [4], done1, done2 from [8]
+  unsigned long long* wave;   // device counters of the two-step kernel: ticket at [0], strip counters from [8], then the flags
+  int* wave_err;              // pinned, device-mapped host word the kernel sets when a wavefront wait timed out
+  int* wave_err_dev;          // its device address
   unsigned long long wave_epoch, wave_tickets;
   unsigned long long strip_count[32];   // host mirror of the device's per-strip completion counters
   unsigned* order_dev;             // launch order table of the two-step kernel
   unsigned order_len;
-  int order_key;                   // (D << 8) | nzf the tables were built for, -1: none
+  long long order_key;             // (D << 32) | nzf the table was built for, -1: none
   int sm_count;
   int resident_blocks;             // co-resident CTAs of lb_resident_kernel on this device (-1: not asked yet)
   int chain_lb;                    // the last launch of this lattice: 1 lb_step_kernel, 2 lb_wave_kernel, 0 anything else
@@ -127,6 +131,14 @@ struct nh_lattice {
 };
 
 namespace {
+
+// A two-step launch whose wavefront stalled has produced garbage: the kernel says so in a host-mapped word, which
+// costs nothing to look at, so every entry point that touches the lattice's state looks (sticky: free the lattice).
+int wave_failed(const nh_lattice* L) {
+  if (L->wave_err && *(volatile int*)L->wave_err)
+    return fail(NH_ECUDA, "two-step LB kernel: a wavefront dependency wait timed out; the lattice's state is invalid");
+  return NH_OK;
+}
 
 constexpr int BLOCK = 256;
 constexpr int NH_EAGAIN = 1;   // internal: this way is not available here, take the plain one
@@ -214,31 +226,22 @@ int launch_lb(nh_lattice* L) {
   const int chained = (L->chain_lb == 1);   // (the Bracket clears it)
   Bracket br(L, KC_LB);
   if (br.rc) return br.rc;
-  constexpr int V = 16 / (int)sizeof(T);
   const int rev = next_sweep(L);
-  if ((L->options & NH_OPT_LB_WIDE) && L->G.nx % V == 0) {
-    const unsigned ngroups = L->G.nfluid / V;
-    nh::lb_step_vec_kernel<T, SH, V><<<blocks_for(ngroups), BLOCK, 0, L->stream>>>(
-        (const T*)L->f[L->cur], (T*)L->f[L->cur ^ 1], (const T*)L->F, L->G, lb_const<T>(L), ngroups, rev);
-  } else {
-    // Consecutive LB steps are chained by programmatic dependent launch: the CTAs of this step may become
-    // resident while the previous step drains (they wait before reading: lb_step_kernel), which hides the
-    // launch latency and the ramp between two short launches (+7 % on 320x320x16, +1 % on 256x256x64).
-    // Only after another lb_step launch of this lattice: next to a kernel with a different shared-memory
-    // carve-out the overlap pins the SMs to that carve-out (measured: 32 400 -> 26 900 MLUPS on config 3).
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(blocks_for(L->G.nfluid)); cfg.blockDim = dim3(BLOCK); cfg.stream = L->stream;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = chained ? 1 : 0;
-    cfg.attrs = at; cfg.numAttrs = 1;
-    NH_CUDA(cudaLaunchKernelEx(&cfg, nh::lb_step_kernel<T, SH>, (const T*)L->f[L->cur], (T*)L->f[L->cur ^ 1],
-                               (const T*)L->F, L->G, lb_const<T>(L), rev));
-    br.end();
-    L->chain_lb = 1;          // cleared by the Bracket of any other launch of this lattice
-    return NH_OK;
-  }
+  // Consecutive LB steps are chained by programmatic dependent launch: the CTAs of this step may become
+  // resident while the previous step drains (they wait before reading: lb_step_kernel), which hides the
+  // launch latency and the ramp between two short launches (+7 % on 320x320x16, +1 % on 256x256x64).
+  // Only after another lb_step launch of this lattice: next to a kernel with a different shared-memory
+  // carve-out the overlap pins the SMs to that carve-out (measured: 32 400 -> 26 900 MLUPS on config 3).
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(blocks_for(L->G.nfluid)); cfg.blockDim = dim3(BLOCK); cfg.stream = L->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = chained ? 1 : 0;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  NH_CUDA(cudaLaunchKernelEx(&cfg, nh::lb_step_kernel<T, SH>, (const T*)L->f[L->cur], (T*)L->f[L->cur ^ 1],
+                             (const T*)L->F, L->G, lb_const<T>(L), rev));
   br.end();
+  L->chain_lb = 1;          // cleared by the Bracket of any other launch of this lattice
   return NH_OK;
 }
 // ---- two LB steps in one launch (nh_lb2.cuh) ----------------------------------------------------
@@ -250,7 +253,7 @@ struct PieceGrid { unsigned YS, nstrips, cps, ppr, rows_per_piece, pieces2; int 
 // (one piece = k warps side by side in one row: nx = 320 -> 160 threads, 384 -> 192, 448 -> 224, 192 -> 96,
 // 576 -> 96 x 3 pieces per row); 0 if there is none.
 int lb2_threads(const nh_lattice* L, int U) {
-  if ((L->options >> 31) & 1) return 128;
+  if (L->tune[NH_TUNE_LB2_THREADS] == 128) return 128;
   const unsigned nx = (unsigned)L->G.nx, pc = 256u * U;
   if (pc % nx == 0 || nx % pc == 0) return 256;
   if (U != 2 || nx % 64) return 256;          // piece_grid will refuse
@@ -264,8 +267,8 @@ bool piece_grid(const nh_lattice* L, int U, PieceGrid* g) {
   if (nx % seg) return false;
   // strips of about 64 K cells per plane (what was measured to pay), or 2^c of them when forced
   unsigned nstrips = 1;
-  const unsigned forced = (L->options >> 27) & 7u;
-  if (forced) nstrips = 1u << forced;
+  const unsigned forced = (unsigned)L->tune[NH_TUNE_LB2_STRIPS];
+  if (forced) nstrips = forced;
   else while (nstrips < (unsigned)nh::WAVE_MAX_STRIPS && ny % (2 * nstrips) == 0 && (size_t)nx * (ny / (2 * nstrips)) >= 65536) nstrips *= 2;
   if (nstrips > (unsigned)nh::WAVE_MAX_STRIPS || ny % nstrips) return false;
   g->nstrips = nstrips;
@@ -288,13 +291,14 @@ bool piece_grid(const nh_lattice* L, int U, PieceGrid* g) {
 }
 int lb2_cells_per_thread(const nh_lattice* L) {
   PieceGrid g;
-  int U = (L->options >> 30) & 1 ? 1 : 2;
-  for (; U >= 1; --U) if (piece_grid(L, U, &g)) return U;
+  int U = L->tune[NH_TUNE_LB2_CELLS] == 1 ? 1 : (L->tune[NH_TUNE_LB2_CELLS] == 4 ? 4 : 2);
+  if (U == 4 && word_of(L->p.precision) == 8) U = 2;      // (four cells per thread only in FP32: registers)
+  for (; U >= 1; U /= 2) if (piece_grid(L, U, &g)) return U;
   return 0;
 }
 // Ring and lead of the wavefront (planes).  Defaults from the B200 measurements in DESIGN.md.
 void lb2_lead(const nh_lattice* L, const PieceGrid& g, int* D, int* R) {
-  *D = (L->options >> 16) & 0xf; *R = (L->options >> 20) & 0x3f;
+  *D = L->tune[NH_TUNE_LB2_LEAD]; *R = L->tune[NH_TUNE_LB2_RING];
   if (*D == 0 && *R == 0) {
     // D = 4, R = 8 where eight ring planes stay within 48 MB of the L2; a shorter wavefront (D = 3, R = 6) for
     // larger strip-planes (measured on 320x320x64: 35 600 against 34 800 MLUPS with the 63 MB ring, 32 600 one-step)
@@ -333,15 +337,15 @@ size_t lb2_max_pieces(int nx, int ny) { return (size_t)nx * (ny + 2) / 128 + ny 
 // every unit after everything it waits for.
 int lb2_order(nh_lattice* L, int D) {
   const int nzf = L->G.nz - 2;
-  const int key = (D << 16) | nzf;
+  const long long key = ((long long)D << 32) | (unsigned)nzf;
   if (L->order_key == key) return NH_OK;
   std::vector<unsigned> o;
   for (int j = 0; j < nzf + D + 1; ++j) {
     const int k2 = j - D - 1;
-    if (k2 >= 0 && k2 < nzf) o.push_back((2u << 16) | (unsigned)k2);
-    if (j < nzf) o.push_back((1u << 16) | (unsigned)j);
+    if (k2 >= 0 && k2 < nzf) o.push_back(0x80000000u | (unsigned)k2);
+    if (j < nzf) o.push_back((unsigned)j);
   }
-  L->order_dev = (unsigned*)(L->wave + 8 + nh::WAVE_MAX_STRIPS + (size_t)nzf * lb2_max_pieces(L->G.nx, L->G.ny));
+  L->order_dev = (unsigned*)(L->wave + 8 + nh::WAVE_MAX_STRIPS + 2 * (size_t)nzf * lb2_max_pieces(L->G.nx, L->G.ny));
   L->order_len = (unsigned)o.size();
   NH_CUDA(cudaMemcpyAsync(L->order_dev, o.data(), o.size() * sizeof(unsigned), cudaMemcpyHostToDevice, L->stream));
   NH_CUDA(cudaStreamSynchronize(L->stream));     // o goes out of scope
@@ -359,12 +363,15 @@ int launch_lb2_u(nh_lattice* L) {
   piece_grid(L, U, &g);
   nh::Wave W;
   W.ticket = L->wave;
-  W.err = (int*)(L->wave + 4);
+  W.err = L->wave_err_dev;
+  // one wait is bounded by about 4 s of SM clocks (nh_debug_tune: milliseconds at a nominal 2 GHz)
+  W.timeout_cycles = L->tune[NH_TUNE_LB2_TIMEOUT_MS] ? 2000000ll * L->tune[NH_TUNE_LB2_TIMEOUT_MS] : 8000000000ll;
+  W.fault = L->tune[NH_TUNE_LB2_FAULT] ? (1ull << 40) : 0ull;
   W.strip_done = L->wave + 8;
   W.YS = g.YS; W.nstrips = g.nstrips; W.cps = g.cps; W.ppr = g.ppr; W.rows_per_piece = g.rows_per_piece;
   W.spr_shift = g.spr_shift;
   W.rplane = (g.YS + 2) * (unsigned)L->G.nx;
-  W.flag1 = (unsigned*)(L->wave + 8 + nh::WAVE_MAX_STRIPS);
+  W.flag1 = L->wave + 8 + nh::WAVE_MAX_STRIPS;
   W.flag2 = W.flag1 + (size_t)nzf * W.cps;
   W.nzf = nzf;
   int D, R;
@@ -376,10 +383,10 @@ int launch_lb2_u(nh_lattice* L) {
   W.units_per_strip = L->order_len * W.cps;
   const unsigned long long units = (unsigned long long)W.units_per_strip * g.nstrips;
   if (units >= 2147483648ull) return fail(NH_EINVAL, "two-step LB kernel: grid too large");
-  if (L->options & NH_OPT_LB_BLOCKORDER) W.ticket = nullptr;
+  if (L->tune[NH_TUNE_LB2_BLOCKORDER]) W.ticket = nullptr;
   W.ticket_base = L->wave_tickets;
   if (W.ticket) L->wave_tickets += units;   // one ticket per CTA
-  W.epoch0 = (unsigned)L->wave_epoch + 1;   // strip s of this launch: epoch0 + s
+  W.epoch0 = L->wave_epoch + 1;             // strip s of this launch: epoch0 + s
   L->wave_epoch += g.nstrips;
   for (unsigned st = 0; st < g.nstrips; ++st) {
     L->strip_count[st] += (unsigned long long)nzf * g.pieces2;
@@ -410,7 +417,10 @@ int launch_lb2_u(nh_lattice* L) {
 }
 template <typename T, bool SH>
 int launch_lb2(nh_lattice* L) {
-  const bool two = lb2_cells_per_thread(L) == 2;
+  const int cells = lb2_cells_per_thread(L);
+  const bool two = cells == 2;
+  if (cells == 4 && sizeof(T) == 4)
+    return lb2_threads(L, 4) == 128 ? launch_lb2_u<T, SH, 4, 128>(L) : launch_lb2_u<T, SH, 4, 256>(L);
   switch (lb2_threads(L, two ? 2 : 1)) {
     case 96: return launch_lb2_u<T, SH, 2, 96>(L);
     case 160: return launch_lb2_u<T, SH, 2, 160>(L);
@@ -426,7 +436,7 @@ int launch_lb2(nh_lattice* L) {
 // cooperative launch is kept out of captures) and not with NH_OPT_LB_ONESTEP (= one launch per LB step).
 template <typename T, bool SH>
 bool resident_usable(nh_lattice* L) {
-  if (L->options & (NH_OPT_LB_ONESTEP | NH_OPT_LB_TWOSTEP | NH_OPT_GRAPH | NH_OPT_LB_WIDE)) return false;
+  if (L->options & (NH_OPT_LB_ONESTEP | NH_OPT_LB_TWOSTEP | NH_OPT_GRAPH)) return false;
   if (L->resident_blocks < 0) {
     int per_sm = 0, coop = 0, dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess ||
@@ -481,7 +491,7 @@ struct TileGrid { dim3 grid; int zchunk; };
 TileGrid tile_grid(const nh_lattice* L) {
   const int tiles = ((L->G.nx + nh::TX - 1) / nh::TX) * ((L->G.ny + nh::TY - 1) / nh::TY);
   const int nzf = L->G.nz - 2;
-  int zchunk = (L->options >> 8) & 0xff;                     // tuning override
+  int zchunk = L->tune[NH_TUNE_FD_PLANES];                   // tuning override
   if (zchunk == 0) {
     int want = (6 * 148 + tiles - 1) / tiles;                // chunks wanted
     int most = (nzf + 7) / 8;                                // chunks of >= 8 planes
@@ -845,12 +855,7 @@ int get_fields_typed(nh_lattice* L, double* rho, double* u, double* n, double* F
   }
   NH_CUDA(cudaGetLastError());
   NH_CUDA(cudaStreamSynchronize(L->stream));
-  if (L->wave_epoch > 0) {   // a two-step launch whose wavefront stalled has produced garbage
-    int werr = 0;
-    NH_CUDA(cudaMemcpy(&werr, L->wave + 4, sizeof(int), cudaMemcpyDeviceToHost));
-    if (werr) return fail(NH_ECUDA, "two-step LB kernel: a wavefront dependency wait timed out");
-  }
-  return NH_OK;
+  return wave_failed(L);       // (the stream is synchronised: a stall in any earlier launch is visible now)
 }
 
 int step_plain(nh_lattice* L, int n_lb, int r);
@@ -918,14 +923,14 @@ namespace {
 
 // rows [y0, y0 + nrows) of a [comps][nz][ny][nx] field <-> a contiguous [comps][nz][nrows][nx] buffer
 template <typename T, bool PACK>
-__global__ void rows_kernel(T* __restrict__ field, T* __restrict__ buf, nh::Geom G, int y0, int nrows) {
-  // blockIdx.y = component * nz + z; the block's threads run along the nrows * nx contiguous words of that plane
+__global__ void rows_kernel(T* __restrict__ field, T* __restrict__ buf, nh::Geom G, int y0, int nrows, unsigned total) {
+  // one thread per word of the buffer; (component * nz + z) and the offset inside that plane's nrows * nx block
+  const unsigned to = blockIdx.x * blockDim.x + threadIdx.x;
+  if (to >= total) return;
   const unsigned per = (unsigned)nrows * G.nx;
-  const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= per) return;
-  const unsigned c = blockIdx.y / G.nz, z = blockIdx.y - c * G.nz;
+  const unsigned cz = to / per, i = to - cz * per;
+  const unsigned c = cz / G.nz, z = cz - c * G.nz;
   const size_t at = (size_t)c * G.N + (size_t)z * G.plane + (size_t)y0 * G.nx + i;   // rows y0.. are contiguous in a plane
-  const size_t to = (size_t)blockIdx.y * per + i;
   if (PACK) buf[to] = field[at];
   else field[at] = buf[to];
 }
@@ -949,8 +954,7 @@ int rows_typed(nh_lattice* L, int field, int y0, int nrows, void* buf) {
   const size_t total = (size_t)comps * L->G.nz * nrows * L->G.nx;
   if (total == 0) return NH_OK;
   Bracket br(L, KC_OTHER);
-  const dim3 grid(blocks_for((size_t)nrows * L->G.nx), (unsigned)(comps * L->G.nz));
-  rows_kernel<T, PACK><<<grid, BLOCK, 0, L->stream>>>((T*)base, (T*)buf, L->G, y0, nrows);
+  rows_kernel<T, PACK><<<blocks_for(total), BLOCK, 0, L->stream>>>((T*)base, (T*)buf, L->G, y0, nrows, (unsigned)total);
   br.end();
   NH_CUDA(cudaGetLastError());
   return NH_OK;
@@ -958,6 +962,7 @@ int rows_typed(nh_lattice* L, int field, int y0, int nrows, void* buf) {
 
 int rows_check(nh_lattice* L, int y0, int nrows, const void* buf) {
   if (!L) return fail(NH_EINVAL, "null handle");
+  { const int rc = wave_failed(L); if (rc) return rc; }
   if (!buf) return fail(NH_EINVAL, "null buffer");
   if (nrows < 0 || y0 < 0 || (long)y0 + nrows > L->G.ny) return fail(NH_EINVAL, "rows outside [0, ny)");
   return NH_OK;
@@ -1009,6 +1014,7 @@ int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_strea
   L->G.N = (size_t)L->G.plane * p->nz;
   L->q0 = p->pitch > 0.0 ? 2.0 * M_PI / p->pitch : 0.0;
   L->stream = (cudaStream_t)cuda_stream;
+  for (int k = 0; k < NH_TUNE_COUNT; ++k) L->tune[k] = 0;
   L->t = 0; L->launches = 0; L->options = 0; L->cur = 0; L->ncur = 0; L->used = 0; L->sweep = 0;
   for (int k = 0; k < KC_COUNT; ++k) { L->ms[k] = 0.0; L->cnt[k] = 0; }
   const size_t N = L->G.N, w = word_of(p->precision);
@@ -1025,9 +1031,15 @@ int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_strea
   L->ring = take((size_t)L->ring_cap * 19 * L->G.nx * (L->G.ny + 2) * w);
   L->wave = (unsigned long long*)take(wave_words(p) * 8);
   L->wave_epoch = 0; L->wave_tickets = 0; L->order_key = -1; L->resident_blocks = -1;
+  L->wave_err = nullptr;
+  e = cudaHostAlloc((void**)&L->wave_err, sizeof(int), cudaHostAllocMapped);
+  if (e != cudaSuccess) { delete L; return cuda_fail(e, "cudaHostAlloc(error word)"); }
+  *L->wave_err = 0;
+  e = cudaHostGetDevicePointer((void**)&L->wave_err_dev, L->wave_err, 0);
+  if (e != cudaSuccess) { cudaFreeHost(L->wave_err); delete L; return cuda_fail(e, "cudaHostGetDevicePointer(error word)"); }
   for (int i = 0; i < 32; ++i) L->strip_count[i] = 0;
   e = cudaMemsetAsync(L->wave, 0, wave_words(p) * 8, L->stream);
-  if (e != cudaSuccess) { delete L; return cuda_fail(e, "cudaMemsetAsync(wave)"); }
+  if (e != cudaSuccess) { cudaFreeHost(L->wave_err); delete L; return cuda_fail(e, "cudaMemsetAsync(wave)"); }
   int rc;
   switch (p->precision) {
     case NH_FP64_SHIFTED: rc = init_typed<double, true>(L); break;
@@ -1035,13 +1047,14 @@ int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_strea
     case NH_FP32_UNSHIFTED: rc = init_typed<float, false>(L); break;
     default: rc = init_typed<double, false>(L); break;
   }
-  if (rc) { delete L; return rc; }
+  if (rc) { cudaFreeHost(L->wave_err); delete L; return rc; }
   *out = L;
   return NH_OK;
 }
 
 int nh_set_director(nh_lattice* L, const double* n_host) {
   if (!L || !n_host) return fail(NH_EINVAL, "null pointer");
+  { const int rc = wave_failed(L); if (rc) return rc; }
   const size_t N = L->G.N;
   NH_CUDA(cudaMemcpyAsync(L->stage, n_host, 3 * N * sizeof(double), cudaMemcpyHostToDevice, L->stream));
   NH_CUDA(cudaMemsetAsync(L->flag, 0, sizeof(int), L->stream));
@@ -1069,6 +1082,7 @@ int nh_set_director(nh_lattice* L, const double* n_host) {
 int nh_step(nh_lattice* L, int n_lb, int n_fd) {
   if (!L) return fail(NH_EINVAL, "null handle");
   if (n_lb < 0) return fail(NH_EINVAL, "n_lb must be >= 0");
+  { const int rc = wave_failed(L); if (rc) return rc; }
   const int r = n_fd < 0 ? L->p.fd_ratio : n_fd;
   if ((L->options & NH_OPT_GRAPH) && n_lb > 0 && !L->defer_force) {
     const int rc = step_graph(L, n_lb, r);
@@ -1113,9 +1127,25 @@ int nh_defer_force(nh_lattice* L, int on) {
 
 int nh_update_force(nh_lattice* L) {
   if (!L) return fail(NH_EINVAL, "null handle");
+  { const int rc = wave_failed(L); if (rc) return rc; }
   const int rc = is_f32(L) ? launch_force<float>(L) : launch_force<double>(L);
   if (rc) return rc;
   NH_CUDA(cudaGetLastError());
+  return NH_OK;
+}
+
+int nh_debug_tune(nh_lattice* L, int key, int value) {
+  if (!L) return fail(NH_EINVAL, "null handle");
+  if (key < 0 || key >= NH_TUNE_COUNT || value < 0) return fail(NH_EINVAL, "unknown tuning key or negative value");
+  if (key == NH_TUNE_LB2_STRIPS && value > nh::WAVE_MAX_STRIPS) return fail(NH_EINVAL, "too many strips");
+  const int rc = drain_events(L);
+  if (rc) return rc;
+  if (!L->graphs.empty()) {                  // captured launches carry the old shapes
+    NH_CUDA(cudaStreamSynchronize(L->stream));
+    for (auto& g : L->graphs) cudaGraphExecDestroy(g.exec);
+    L->graphs.clear();
+  }
+  L->tune[key] = value;
   return NH_OK;
 }
 
@@ -1135,6 +1165,8 @@ int nh_kernel_time(nh_lattice* L, int which, double* ms_total, long* launches) {
   if (!L || which < 0 || which >= KC_COUNT) return fail(NH_EINVAL, "bad arguments");
   int rc = drain_events(L);
   if (rc) return rc;
+  rc = wave_failed(L);
+  if (rc) return rc;
   if (ms_total) *ms_total = L->ms[which];
   if (launches) *launches = L->cnt[which];
   return NH_OK;
@@ -1144,6 +1176,7 @@ void nh_free(nh_lattice* L) {
   if (!L) return;
   for (auto& pr : L->pool) { cudaEventDestroy(pr.a); cudaEventDestroy(pr.b); }
   for (auto& g : L->graphs) cudaGraphExecDestroy(g.exec);
+  if (L->wave_err) cudaFreeHost(L->wave_err);
   delete L;
 }
 

@@ -45,13 +45,15 @@ constexpr int WAVE_MAX_STRIPS = 32;
 
 struct Wave {
   unsigned long long* ticket;     // device counter, never reset
-  unsigned* flag1;                // [nzf][cps] strip number (epoch) of the last finished phase-1 unit
-  unsigned* flag2;                // the same for phase 2
+  unsigned long long* flag1;      // [nzf][cps] strip number (epoch) of the last finished phase-1 unit
+  unsigned long long* flag2;      // the same for phase 2
   unsigned long long* strip_done; // [nstrips] finished phase-2 units per strip, never reset
-  int* err;                       // set to 1 if a wait timed out
+  volatile int* err;              // HOST-mapped word, set to 1 if a wait timed out (read by every API entry)
+  long long timeout_cycles;       // bound of one wait, in SM clocks
+  unsigned long long fault;       // test hook (nh_debug_tune): added to the epoch the waits ask for, so that they cannot be met
   unsigned long long ticket_base; // value of *ticket when this launch starts
   unsigned long long strip_target[WAVE_MAX_STRIPS];  // value of strip_done[s] when strip s of THIS launch is done
-  unsigned epoch0;                // flags of strip s of this launch carry epoch0 + s (> 0, grows across launches)
+  unsigned long long epoch0;      // flags of strip s of this launch carry epoch0 + s (> 0, grows across launches; 64 bits: never wraps)
   int nzf;                        // fluid planes
   unsigned YS;                    // lattice rows per strip (ny = nstrips * YS)
   unsigned nstrips;
@@ -64,17 +66,11 @@ struct Wave {
   int D;                          // lead of phase 1 over phase 2, in planes (>= 1)
   int R;                          // ring slots (planes), R >= D + 2
   int reverse;                    // sweep from the top plate down
-  const unsigned* order;          // [order_len] (phase << 16) | logical plane, in launch order
+  const unsigned* order;          // [order_len] logical plane, bit 31 set for phase 2, in launch order
 };
 
 // p[i] = start of direction i inside a population array
 template <typename T> struct DirTab { T* p[Q]; };
-
-__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
-  unsigned v;
-  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
 
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
   unsigned long long v;
@@ -115,8 +111,8 @@ __device__ __forceinline__ bool deps_ready(const Wave& W, int phase, int k, unsi
         unsigned pq = q + dq;                                      // periodic along x, no division
         pq = (pq == 0) ? W.ppr - 1 : pq - 1;
         if (pq == W.ppr) pq = 0;
-        const unsigned* f = (phase == 2 ? W.flag1 : W.flag2) + (size_t)j * W.cps + (unsigned)p * W.ppr + pq;
-        ok = ld_acquire_u32(f) >= W.epoch0 + strip;
+        const unsigned long long* f = (phase == 2 ? W.flag1 : W.flag2) + (size_t)j * W.cps + (unsigned)p * W.ppr + pq;
+        ok = ld_acquire_u64(f) >= W.epoch0 + strip + W.fault;
       }
     }
   } else if (lane == 27 && phase == 1 && strip > 0 && k < W.R) {
@@ -199,7 +195,8 @@ __device__ __forceinline__ void gather_cells(const Tab& S, unsigned zm, unsigned
 // its flags (the old readers of its ring slot) only before it stores; a phase-2 unit checks before
 // it gathers.  One barrier at the end, then thread 0 publishes the unit (fence, flag, counter).
 template <typename T, bool SHIFTED, int U, int NT>
-__global__ void __launch_bounds__(NT, (sizeof(T) == 4 ? 1024 : (U == 2 ? 256 : 512)) / NT)
+__global__ void __launch_bounds__(NT, ((sizeof(T) == 4 ? (U == 4 ? 512 : (U == 1 ? 1536 : 1024)) : (U == 2 ? 256 : 512)) / NT) > 0
+                                          ? (sizeof(T) == 4 ? (U == 4 ? 512 : (U == 1 ? 1536 : 1024)) : (U == 2 ? 256 : 512)) / NT : 1)
 lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restrict__ Flc,
                Geom G, LbConst<T> C, Wave W) {
   const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -216,7 +213,7 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
     const unsigned rem = tk - st * W.units_per_strip;
     const unsigned unit = rem / W.cps, piece = rem - unit * W.cps;
     const unsigned code = W.order[unit];
-    ph = (int)(code >> 16); kk = (int)(code & 0xffffu);
+    ph = (code >> 31) ? 2 : 1; kk = (int)(code & 0x7fffffffu);
     pr = piece / W.ppr; qq = piece - pr * W.ppr;
   };
   if (W.ticket) {                       // safe order: a ticket drawn when the CTA starts to run
@@ -244,7 +241,11 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
     while (!deps_ready(W, phase, k, strip, prow, q, lane)) {
       __nanosleep(ns);
       if (ns < 512) ns *= 2;
-      if (clock64() - t0 > 8000000000ll) { if (lane == 0) atomicExch(W.err, 1); break; }
+      // give up after the bound, or at once when another CTA already has: the launch then ends quickly and every
+      // later API call on this lattice reports the error (nh_api.cu: wave_failed)
+      const long long waited = clock64() - t0;
+      if (waited > 2000000ll && *W.err) break;          // (the word lives in host memory: not looked at before ~1 ms)
+      if (waited > W.timeout_cycles) { if (lane == 0) { *W.err = 1; __threadfence_system(); } break; }
     }
   };
   const unsigned nx = (unsigned)G.nx, ny = (unsigned)G.ny;
@@ -311,8 +312,8 @@ lb_wave_kernel(DirTab<const T> A, DirTab<T> ring, DirTab<T> B, const T* __restri
   if (threadIdx.x == 0) {
     // publish: everything this CTA read and wrote is ordered before the flag (and the strip counter)
     __threadfence();
-    unsigned* f = (phase == 1 ? W.flag1 : W.flag2) + (size_t)k * W.cps + prow * W.ppr + q;
-    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(f), "r"(W.epoch0 + strip) : "memory");
+    unsigned long long* f = (phase == 1 ? W.flag1 : W.flag2) + (size_t)k * W.cps + prow * W.ppr + q;
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(f), "l"(W.epoch0 + strip) : "memory");
     if (phase == 2) asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(W.strip_done + strip), "l"(1ull) : "memory");
   }
 }

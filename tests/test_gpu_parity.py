@@ -247,7 +247,7 @@ def test_options_do_not_change_results():
     """Scheduling / kernel-variant switches are bit-neutral or within round-off of each other."""
     m = nh()
     ref = None
-    for opt in (0, m.OPT_TIMING, m.OPT_GRAPH, m.OPT_FD_DIRECT, m.OPT_LB_WIDE, m.OPT_FD_DIRECT | m.OPT_LB_WIDE):
+    for opt in (0, m.OPT_TIMING, m.OPT_GRAPH, m.OPT_FD_DIRECT, m.OPT_FD_NOVEC, m.OPT_FD_DIRECT | m.OPT_NO_SERPENTINE):
         p = I.config(0, fd_ratio=3)
         d = p.pop("director")
         p.pop("steps")
@@ -298,9 +298,10 @@ def test_two_step_kernel_is_bit_identical(shape, r):
     d = I.noisy_homeotropic(nx, ny, nz, 0.1)
     p = dict(nx=nx, ny=ny, nz=nz, tau=0.7, K=0.015, pitch=9.0, xi=0.8, gamma1=1.3, g=(2e-6, -1e-6, 1.5e-6), fd_ratio=r)
 
-    def run(precision, opt, chunks):
+    def run(precision, opt, chunks, **knobs):
         g = m.Lattice(**dict(p, precision=precision))
         g.set_options(opt)
+        g.debug_tune(**knobs)
         g.set_director(d)
         for c in chunks:
             g.step(c)
@@ -309,14 +310,47 @@ def test_two_step_kernel_is_bit_identical(shape, r):
         return f
 
     T = m.OPT_LB_TWOSTEP
+    variants = [(T, {}), (T | m.OPT_NO_SERPENTINE, {}), (T, dict(lb2_cells=1)), (T, dict(lb2_threads=128)),
+                (T, dict(lb2_lead=1, lb2_ring=3)), (T, dict(lb2_lead=3, lb2_ring=12, lb2_blockorder=1)),
+                (T, dict(lb2_blockorder=1, lb2_cells=1)), (T, dict(lb2_strips=2)),
+                (T, dict(lb2_strips=4, lb2_lead=2, lb2_ring=5)), (T, dict(lb2_strips=8, lb2_blockorder=1))]
     for precision in (0, 1):
         ref = run(precision, m.OPT_LB_ONESTEP, [43])
-        for opt in (T, T | m.OPT_NO_SERPENTINE, T | (1 << 30), T | (1 << 31), T | (1 << 16) | (3 << 20),
-                    T | (3 << 16) | (12 << 20) | m.OPT_LB_BLOCKORDER, T | m.OPT_LB_BLOCKORDER | (1 << 30),
-                    T | (1 << 27), T | (2 << 27) | (2 << 16) | (5 << 20), T | (3 << 27) | m.OPT_LB_BLOCKORDER):   # 2, 4, 8 strips
-            f = run(precision, opt, [1, 7, 20, 15])
+        for opt, knobs in variants:
+            if ny % knobs.get("lb2_strips", 1):
+                continue                      # (the number of strips must divide ny)
+            f = run(precision, opt, [1, 7, 20, 15], **knobs)
             for k in ref:
-                assert np.array_equal(ref[k], f[k]), (shape, precision, hex(opt), k)
+                assert np.array_equal(ref[k], f[k]), (shape, precision, hex(opt), knobs, k)
+
+
+def test_wavefront_timeout_is_reported_by_the_next_calls():
+    """A dependency wait of the two-step LB kernel that is not met within its bound ends the launch and makes
+    every later call on the lattice fail with NH_ECUDA -- nh_step included, not only nh_get_fields.  Forced with
+    the test hook that makes the waits ask for an epoch that never comes (include/nh_debug.h)."""
+    m = nh()
+    p = I.config(1, nx=64, ny=32, nz=14, fd_ratio=4)
+    d = p.pop("director")
+    p.pop("steps")
+    g = m.Lattice(**dict(p, precision=1))
+    g.set_options(m.OPT_LB_TWOSTEP)
+    g.set_director(d)
+    g.step(8)
+    g.get_fields()                                      # fine so far
+    g.debug_tune(lb2_fault=1, lb2_timeout_ms=20)
+    g.step(2)                                           # asynchronous: this call cannot know yet
+    g.synchronize()
+    for call in (lambda: g.step(2), lambda: g.get_fields(), lambda: g.update_force(), lambda: g.set_director(d)):
+        with pytest.raises(m.NhError) as ei:
+            call()
+        assert ei.value.code == -3 and "wavefront" in str(ei.value)
+    g.close()
+    # another lattice is unaffected
+    h = m.Lattice(**dict(p, precision=1))
+    h.set_options(m.OPT_LB_TWOSTEP)
+    h.set_director(d)
+    h.step(8)
+    h.get_fields()
 
 
 def test_config3_full_size_bench_configuration():
