@@ -10,8 +10,9 @@ One bench "step" is one pass over every row of the hot path: r LB steps (collide
 then the velocity store, predictor, corrector and force update.  MLUPS = fluid cells x LB steps /
 seconds / 1e6 (reading G21).
 
-Prints ONE JSON line (rank 0).  Multi-GPU: the path is not sharded ("replicas only"):
---gpus N runs N independent replicas, one per rank, and reports their summed throughput.
+Prints ONE JSON line (rank 0).  Multi-GPU (--gpus N, under torchrun or started by bench.py itself): ONE lattice of N
+times the config's rows, cut into N y-slabs, one per rank, halo rows exchanged over NCCL (weak scaling; DESIGN.md
+section 8); --replicas runs N independent lattices instead.
 """
 from __future__ import annotations
 
@@ -53,10 +54,12 @@ def parse():
     ap.add_argument("--frank3", action="store_true",
                     help="three-constant Frank energy (row f2): K11 = K, K22 : K33 in the ratios of the paper's Table 1")
     ap.add_argument("--slabs", type=int, default=0,
-                    help="row f4: ONE lattice cut into y-slabs with halo exchange (paper_2503_06610_b200/slabs.py) instead of "
-                         "independent replicas.  Under torchrun: one slab per rank over NCCL, the config's ny rows PER RANK "
-                         "(weak scaling; the value is ignored).  On one GPU: the config's lattice cut into this many slabs "
-                         "held by one process (measures the decomposition's overhead)")
+                    help="ONE lattice cut into y-slabs with halo exchange (paper_2503_06610_b200/slabs.py).  With more than one "
+                         "GPU this is the default: one slab per rank over NCCL, the config's ny rows PER RANK (weak scaling; the "
+                         "value is ignored).  On one GPU: the config's lattice cut into this many slabs held by one process "
+                         "(measures the decomposition's overhead)")
+    ap.add_argument("--replicas", action="store_true",
+                    help="with more than one GPU: N independent lattices, one per rank, no communication, instead of slabs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the sustained (>= 3 s) loop and the fp64 / one_step sub-records")
@@ -324,6 +327,15 @@ def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not launched by torchrun: start the N ranks ourselves (one process per GPU, NCCL over NVLink)
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
 
     import torch
     import torch.distributed as dist
@@ -341,12 +353,16 @@ def main():
     torch.cuda.set_stream(torch.cuda.Stream())
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if rank == 0:
+            sys.stderr.write("bench.py: communicator backend=%s nranks=%d (NCCL_DEBUG=INFO shows its rings and NVLS)\n"
+                             % (dist.get_backend(), dist.get_world_size()))
     if rank == 0:
         nh_build.build()
     if world > 1:
         dist.barrier()
 
-    if args.slabs:
+    # more than one GPU: the path shards as y-slabs with a halo exchange; --replicas opts out
+    if args.slabs or (world > 1 and not args.replicas):
         return run_slabs(args, world, rank, local)
 
     p, d, desc = workload(args)

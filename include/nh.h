@@ -174,6 +174,12 @@ size_t nh_rows_bytes(const nh_lattice* L, int field, int nrows);
 int nh_get_rows(nh_lattice* L, int field, int y0, int nrows, void* dev_buf);
 int nh_set_rows(nh_lattice* L, int field, int y0, int nrows, const void* dev_buf);
 
+/* The same for TWO row ranges in one launch -- a slab's two edges, or its two halos: rows [y0_a, y0_a + nrows)
+ * go to / come from the first half of `dev_buf`, rows [y0_b, y0_b + nrows) the second half; each half is laid out
+ * like the buffer of nh_get_rows (2 x nh_rows_bytes(L, field, nrows) bytes in all). */
+int nh_get_rows_pair(nh_lattice* L, int field, int y0_a, int y0_b, int nrows, void* dev_buf);
+int nh_set_rows_pair(nh_lattice* L, int field, int y0_a, int y0_b, int nrows, const void* dev_buf);
+
 /* Recompute F^LC (Eq. 12) from the director and the stored velocity now in the lattice -- the force
  * step of nh_step on its own, for use after the director's (and, with Leslie viscosities, the
  * velocity's) halo rows have been refreshed.  Asynchronous on the lattice's stream. */

@@ -23,7 +23,8 @@ KERNEL_CLASSES = ("lb", "velocity", "predictor", "corrector", "force", "other", 
 
 EXPORTS = ("nh_workspace_bytes", "nh_init_lattice", "nh_set_director", "nh_step", "nh_get_fields",
            "nh_time", "nh_launch_count", "nh_set_options", "nh_kernel_time", "nh_free", "nh_last_error",
-           "nh_rows_bytes", "nh_get_rows", "nh_set_rows", "nh_update_force", "nh_defer_force", "nh_debug_tune")
+           "nh_rows_bytes", "nh_get_rows", "nh_set_rows", "nh_update_force", "nh_defer_force", "nh_debug_tune",
+           "nh_get_rows_pair", "nh_set_rows_pair")
 
 
 class NhParams(C.Structure):
@@ -73,6 +74,8 @@ def load():
         lib.nh_rows_bytes.restype = C.c_size_t
         lib.nh_get_rows.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
         lib.nh_set_rows.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
+        lib.nh_get_rows_pair.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
+        lib.nh_set_rows_pair.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
         lib.nh_update_force.argtypes = [C.c_void_p]
         lib.nh_defer_force.argtypes = [C.c_void_p, C.c_int]
         lib.nh_debug_tune.argtypes = [C.c_void_p, C.c_int, C.c_int]
@@ -202,6 +205,15 @@ class Lattice:
     def set_rows(self, field, y0, nrows, buf):
         assert buf.is_cuda and buf.is_contiguous() and buf.numel() * buf.element_size() >= self.rows_bytes(field, nrows)
         _check(load().nh_set_rows(self._h, FIELDS.index(field), int(y0), int(nrows), buf.data_ptr()))
+
+    def get_rows_pair(self, field, y0_a, y0_b, nrows, buf):
+        """Rows [y0_a, +nrows) and [y0_b, +nrows) into the two halves of `buf` (2 x rows_bytes), one launch."""
+        assert buf.is_cuda and buf.is_contiguous() and buf.numel() * buf.element_size() >= 2 * self.rows_bytes(field, nrows)
+        _check(load().nh_get_rows_pair(self._h, FIELDS.index(field), int(y0_a), int(y0_b), int(nrows), buf.data_ptr()))
+
+    def set_rows_pair(self, field, y0_a, y0_b, nrows, buf):
+        assert buf.is_cuda and buf.is_contiguous() and buf.numel() * buf.element_size() >= 2 * self.rows_bytes(field, nrows)
+        _check(load().nh_set_rows_pair(self._h, FIELDS.index(field), int(y0_a), int(y0_b), int(nrows), buf.data_ptr()))
 
     def update_force(self):
         _check(load().nh_update_force(self._h))

@@ -16,6 +16,7 @@
 
 #include "nh_fd.cuh"
 #include "nh_fd_tile.cuh"
+#include "nh_fd_vec.cuh"
 #include "nh_frank3.cuh"
 #include "nh_lb.cuh"
 #include "nh_lb2.cuh"
@@ -512,6 +513,47 @@ bool tiles_fit(const nh_lattice* L) {
   return g.grid.y <= 65535u && g.grid.z <= 65535u;
 }
 
+// ---- four cells per thread along x (nh_fd_vec.cuh): FP32, rows a multiple of 64 cells ----------------------
+template <typename T>
+bool vec_usable(const nh_lattice* L) {
+  return sizeof(T) == 4 && L->G.nx % nh::VW == 0 && !(L->options & (NH_OPT_FD_DIRECT | NH_OPT_FD_NOVEC)) &&
+         (L->G.ny + nh::VTY - 1) / nh::VTY <= 65535;
+}
+// z-chunks of the march: the number of chunks per tile that minimises (waves of CTAs) x (planes per chunk + the
+// `prime` planes a chunk stages before its first result), with `per_sm` CTAs resident per SM
+TileGrid vec_grid(const nh_lattice* L, int per_sm, int prime) {
+  const int tx = L->G.nx / nh::VW, ty = (L->G.ny + nh::VTY - 1) / nh::VTY, tiles = tx * ty;
+  const int nzf = L->G.nz - 2;
+  const long slots = (long)(per_sm < 1 ? 1 : per_sm) * L->sm_count;
+  int best = 1;
+  long best_cost = -1;
+  for (int c = 1; c <= nzf && c <= 65535; ++c) {
+    const int planes = (nzf + c - 1) / c;
+    if (c > 1 && planes < 4) break;
+    const long ctas = (long)tiles * ((nzf + planes - 1) / planes);
+    const long cost = ((ctas + slots - 1) / slots) * (planes + prime);
+    if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = planes; }
+  }
+  TileGrid g;
+  g.zchunk = L->tune[NH_TUNE_FD_PLANES] ? L->tune[NH_TUNE_FD_PLANES] : best;
+  if (g.zchunk > nzf) g.zchunk = nzf;
+  g.grid = dim3((unsigned)tx, (unsigned)ty, (unsigned)((nzf + g.zchunk - 1) / g.zchunk));
+  return g;
+}
+template <typename T, int STAGE>
+int launch_director_vec(nh_lattice* L, const nh::FdConst<T>& C, int with_flow, const T* field, const T* a_in, T* out, T* a_out, int cls) {
+  Bracket br(L, cls);
+  if (br.rc) return br.rc;
+  const size_t sm = nh::director_vec_smem_bytes<T>();
+  int per_sm = 0;
+  NH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, nh::director_vec_kernel<T, STAGE>, nh::VTHREADS, sm));
+  const TileGrid g = vec_grid(L, per_sm, 2);
+  nh::director_vec_kernel<T, STAGE><<<g.grid, nh::VTHREADS, sm, L->stream>>>(field, (const T*)L->u, a_in, out, a_out, L->G, C,
+                                                                            with_flow, g.zchunk);
+  br.end();
+  return NH_OK;
+}
+
 // ---- three-constant Frank energy (nh_frank3.cuh) ------------------------------------------------
 template <typename T>
 nh::Frank3<T> frank3_const(const nh_lattice* L) {
@@ -677,6 +719,16 @@ int launch_director(nh_lattice* L, int r) {
     L->ncur ^= 1;
     return mirror_plates<T>(L, L->n[L->ncur]);
   }
+  if (tiled && vec_usable<T>(L)) {
+    int rc = launch_director_vec<T, 0>(L, C, with_flow, (const T*)L->n[L->ncur], nullptr, (T*)L->nP, (T*)L->a, KC_PRED);
+    if (rc) return rc;
+    rc = mirror_plates<T>(L, L->nP);
+    if (rc) return rc;
+    rc = launch_director_vec<T, 1>(L, C, with_flow, (const T*)L->nP, (const T*)L->a, (T*)L->n[L->ncur ^ 1], nullptr, KC_CORR);
+    if (rc) return rc;
+    L->ncur ^= 1;
+    return mirror_plates<T>(L, L->n[L->ncur]);
+  }
   {
     Bracket br(L, KC_PRED);
     if (br.rc) return br.rc;
@@ -716,6 +768,8 @@ int enable_tile_smem() {
   const int db = (int)nh::director_smem_bytes<T>(), fb = (int)nh::force_smem_bytes<T, false>();
   const int fvb = (int)nh::force_smem_bytes<T, true>();
   const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+  NH_CUDA(cudaFuncSetAttribute(nh::director_vec_kernel<T, 0>, attr, (int)nh::director_vec_smem_bytes<T>()));
+  NH_CUDA(cudaFuncSetAttribute(nh::director_vec_kernel<T, 1>, attr, (int)nh::director_vec_smem_bytes<T>()));
   NH_CUDA(cudaFuncSetAttribute(nh::director_tile_kernel<T, 0, true>, attr, db));
   NH_CUDA(cudaFuncSetAttribute(nh::director_tile_kernel<T, 1, true>, attr, db));
   NH_CUDA(cudaFuncSetAttribute(nh::director_tile_kernel<T, 0, false>, attr, db));
@@ -922,15 +976,19 @@ int step_graph(nh_lattice* L, int n_lb, int r) {
 namespace {
 
 // rows [y0, y0 + nrows) of a [comps][nz][ny][nx] field <-> a contiguous [comps][nz][nrows][nx] buffer
+// rows [y0a, y0a + nrows) and, in the second half of the buffer, rows [y0b, y0b + nrows) of a [comps][nz][ny][nx]
+// field <-> a contiguous [2][comps][nz][nrows][nx] buffer (`half` = words of one half; one range only: total = half)
 template <typename T, bool PACK>
-__global__ void rows_kernel(T* __restrict__ field, T* __restrict__ buf, nh::Geom G, int y0, int nrows, unsigned total) {
+__global__ void rows_kernel(T* __restrict__ field, T* __restrict__ buf, nh::Geom G, int y0a, int y0b, int nrows,
+                            unsigned half, unsigned total) {
   // one thread per word of the buffer; (component * nz + z) and the offset inside that plane's nrows * nx block
   const unsigned to = blockIdx.x * blockDim.x + threadIdx.x;
   if (to >= total) return;
+  const unsigned second = to >= half ? 1u : 0u, w = to - second * half;
   const unsigned per = (unsigned)nrows * G.nx;
-  const unsigned cz = to / per, i = to - cz * per;
+  const unsigned cz = w / per, i = w - cz * per;
   const unsigned c = cz / G.nz, z = cz - c * G.nz;
-  const size_t at = (size_t)c * G.N + (size_t)z * G.plane + (size_t)y0 * G.nx + i;   // rows y0.. are contiguous in a plane
+  const size_t at = (size_t)c * G.N + (size_t)z * G.plane + (size_t)(second ? y0b : y0a) * G.nx + i;   // rows are contiguous in a plane
   if (PACK) buf[to] = field[at];
   else field[at] = buf[to];
 }
@@ -946,15 +1004,15 @@ int field_of(nh_lattice* L, int field, void** base, int* comps) {
 }
 
 template <typename T, bool PACK>
-int rows_typed(nh_lattice* L, int field, int y0, int nrows, void* buf) {
+int rows_typed(nh_lattice* L, int field, int y0a, int y0b, int ranges, int nrows, void* buf) {
   void* base = nullptr;
   int comps = 0;
   const int rc = field_of(L, field, &base, &comps);
   if (rc) return rc;
-  const size_t total = (size_t)comps * L->G.nz * nrows * L->G.nx;
+  const size_t half = (size_t)comps * L->G.nz * nrows * L->G.nx, total = half * ranges;
   if (total == 0) return NH_OK;
   Bracket br(L, KC_OTHER);
-  rows_kernel<T, PACK><<<blocks_for(total), BLOCK, 0, L->stream>>>((T*)base, (T*)buf, L->G, y0, nrows, (unsigned)total);
+  rows_kernel<T, PACK><<<blocks_for(total), BLOCK, 0, L->stream>>>((T*)base, (T*)buf, L->G, y0a, y0b, nrows, (unsigned)half, (unsigned)total);
   br.end();
   NH_CUDA(cudaGetLastError());
   return NH_OK;
@@ -1108,15 +1166,31 @@ size_t nh_rows_bytes(const nh_lattice* L, int field, int nrows) {
 int nh_get_rows(nh_lattice* L, int field, int y0, int nrows, void* dev_buf) {
   const int rc = rows_check(L, y0, nrows, dev_buf);
   if (rc) return rc;
-  return is_f32(L) ? rows_typed<float, true>(L, field, y0, nrows, dev_buf)
-                   : rows_typed<double, true>(L, field, y0, nrows, dev_buf);
+  return is_f32(L) ? rows_typed<float, true>(L, field, y0, 0, 1, nrows, dev_buf)
+                   : rows_typed<double, true>(L, field, y0, 0, 1, nrows, dev_buf);
 }
 
 int nh_set_rows(nh_lattice* L, int field, int y0, int nrows, const void* dev_buf) {
   const int rc = rows_check(L, y0, nrows, dev_buf);
   if (rc) return rc;
-  return is_f32(L) ? rows_typed<float, false>(L, field, y0, nrows, const_cast<void*>(dev_buf))
-                   : rows_typed<double, false>(L, field, y0, nrows, const_cast<void*>(dev_buf));
+  return is_f32(L) ? rows_typed<float, false>(L, field, y0, 0, 1, nrows, const_cast<void*>(dev_buf))
+                   : rows_typed<double, false>(L, field, y0, 0, 1, nrows, const_cast<void*>(dev_buf));
+}
+
+int nh_get_rows_pair(nh_lattice* L, int field, int y0_a, int y0_b, int nrows, void* dev_buf) {
+  int rc = rows_check(L, y0_a, nrows, dev_buf);
+  if (!rc) rc = rows_check(L, y0_b, nrows, dev_buf);
+  if (rc) return rc;
+  return is_f32(L) ? rows_typed<float, true>(L, field, y0_a, y0_b, 2, nrows, dev_buf)
+                   : rows_typed<double, true>(L, field, y0_a, y0_b, 2, nrows, dev_buf);
+}
+
+int nh_set_rows_pair(nh_lattice* L, int field, int y0_a, int y0_b, int nrows, const void* dev_buf) {
+  int rc = rows_check(L, y0_a, nrows, dev_buf);
+  if (!rc) rc = rows_check(L, y0_b, nrows, dev_buf);
+  if (rc) return rc;
+  return is_f32(L) ? rows_typed<float, false>(L, field, y0_a, y0_b, 2, nrows, const_cast<void*>(dev_buf))
+                   : rows_typed<double, false>(L, field, y0_a, y0_b, 2, nrows, const_cast<void*>(dev_buf));
 }
 
 int nh_defer_force(nh_lattice* L, int on) {

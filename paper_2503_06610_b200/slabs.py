@@ -89,8 +89,9 @@ class HaloSchedule:
         self.valid_f = self.H
 
     def refresh(self, actions):
+        """Only the outermost H - valid_f halo rows have gone stale: those are the rows that travel."""
         if self.valid_f < self.H:
-            actions.append(("exchange", "populations"))
+            actions.append(("exchange", "populations", self.H - max(self.valid_f, 0)))
             self.valid_f = self.H
 
     def after_director(self, actions):
@@ -180,54 +181,79 @@ class SlabLattice:
 
     # ---- halo exchange -------------------------------------------------------------------------------
     def _buffers(self, s, field):
+        """Per slab and field: `send` = [rows for the slab below | rows for the slab above], `recv` = [rows from the
+        slab below | rows from the slab above]; each half holds up to H packed rows."""
         key = (s, field)
         if key not in self._buf:
             lat = self.local[s]
-            self._buf[key] = {k: lat.new_rows_buffer(field, self.H) for k in ("send_lo", "send_hi", "recv_lo", "recv_hi")}
+            half = lat.rows_bytes(field, self.H)
+            self._buf[key] = {k: lat.new_rows_buffer(field, 2 * self.H) for k in ("send", "recv")}
+            self._buf[key]["half"] = half
         return self._buf[key]
 
-    def exchange(self, field):
-        """Refresh the 2 x H halo rows of `field` on every slab from its two neighbours' edge rows."""
+    def _on_stream(self, lat):
+        """Everything an exchange enqueues must be ordered with the lattice's own launches: make the lattice's stream
+        torch's current stream for the duration (torch copies and NCCL then wait on it, whatever the ambient stream)."""
+        import contextlib
+        st = getattr(lat, "_stream", None)
+        if st is None:
+            return contextlib.nullcontext()
+        import torch
+        return torch.cuda.stream(st)
+
+    def exchange(self, field, m=None):
+        """Refresh the outermost `m` (default: all H) rows of both halos of `field` on every slab from its two
+        neighbours.  One pack launch and one unpack launch per slab (both faces at once)."""
         H = self.H
+        m = H if m is None else int(m)
+        assert 1 <= m <= H
         for s, lat in self.local.items():
             rows = self.parts[s][1]
             b = self._buffers(s, field)
-            lat.get_rows(field, H, H, b["send_lo"])            # my first H rows -> the slab below, its upper halo
-            lat.get_rows(field, rows, H, b["send_hi"])         # my last H rows  -> the slab above, its lower halo
+            with self._on_stream(lat):
+                # first half: my first owned rows that the slab below lacks at the far end of its upper halo;
+                # second half: my last owned rows that the slab above lacks at the far end of its lower halo
+                lat.get_rows_pair(field, 2 * H - m, rows, m, b["send"])
         if self.group is None or self.size == 1:
             for s, lat in self.local.items():
                 rows = self.parts[s][1]
                 lo, hi = (s - 1) % self.size, (s + 1) % self.size
-                lat.set_rows(field, 0, H, self._buffers(lo, field)["send_hi"])
-                lat.set_rows(field, H + rows, H, self._buffers(hi, field)["send_lo"])
+                nb = lat.rows_bytes(field, m)
+                with self._on_stream(lat):
+                    if lo == s and hi == s:      # one slab, its own neighbour on both sides: its two halves, swapped
+                        lat.set_rows_pair(field, 2 * H + rows - m, 0, m, self._buffers(s, field)["send"])
+                    else:
+                        lat.set_rows(field, 0, m, self._buffers(lo, field)["send"][nb:2 * nb])
+                        lat.set_rows(field, 2 * H + rows - m, m, self._buffers(hi, field)["send"][:nb])
         else:
             import torch.distributed as dist
             s = self.rank
             lat, rows, b = self.local[s], self.parts[s][1], self._buffers(s, field)
+            nb = lat.rows_bytes(field, m)
             lo = dist.get_global_rank(self.group, (s - 1) % self.size)
             hi = dist.get_global_rank(self.group, (s + 1) % self.size)
-            # Same order on every rank.  With two ranks both neighbours are the same peer and messages between a
-            # pair match in posting order: my first send (lower edge) meets the peer's first receive (its upper halo).
-            staged = b["send_lo"].is_cuda and dist.get_backend(self.group) == "gloo"
-            w = {k: v.cpu() for k, v in b.items()} if staged else b    # gloo moves host memory only: stage through it
-            ops = [dist.P2POp(dist.isend, w["send_lo"], lo, self.group),
-                   dist.P2POp(dist.isend, w["send_hi"], hi, self.group),
-                   dist.P2POp(dist.irecv, w["recv_hi"], hi, self.group),
-                   dist.P2POp(dist.irecv, w["recv_lo"], lo, self.group)]
-            for req in dist.batch_isend_irecv(ops):
-                req.wait()
-            if staged:
-                b["recv_lo"].copy_(w["recv_lo"])
-                b["recv_hi"].copy_(w["recv_hi"])
-            lat.set_rows(field, 0, H, b["recv_lo"])
-            lat.set_rows(field, H + rows, H, b["recv_hi"])
+            with self._on_stream(lat):
+                # Same order on every rank.  With two ranks both neighbours are the same peer and messages between a
+                # pair match in posting order: my first send (to below) meets the peer's first receive (from above).
+                staged = b["send"].is_cuda and dist.get_backend(self.group) == "gloo"
+                send = b["send"][:2 * nb].cpu() if staged else b["send"]      # gloo moves host memory only
+                recv = send.new_empty(2 * nb) if staged else b["recv"]
+                ops = [dist.P2POp(dist.isend, send[:nb], lo, self.group),
+                       dist.P2POp(dist.isend, send[nb:2 * nb], hi, self.group),
+                       dist.P2POp(dist.irecv, recv[nb:2 * nb], hi, self.group),
+                       dist.P2POp(dist.irecv, recv[:nb], lo, self.group)]
+                for req in dist.batch_isend_irecv(ops):
+                    req.wait()
+                if staged:
+                    b["recv"][:2 * nb].copy_(recv)
+                lat.set_rows_pair(field, 0, 2 * H + rows - m, m, b["recv"])
         self.exchanges += 1
-        self.bytes_sent += sum(2 * lat.rows_bytes(field, H) for lat in self.local.values())
+        self.bytes_sent += sum(2 * lat.rows_bytes(field, m) for lat in self.local.values())
 
     def _run(self, actions):
         for a in actions:
             if a[0] == "exchange":
-                self.exchange(a[1])
+                self.exchange(*a[1:])
             elif a[0] == "step":
                 for lat in self.local.values():
                     lat.step(a[1], a[2])

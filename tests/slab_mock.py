@@ -90,11 +90,21 @@ class MockLattice:
 
     def get_rows(self, field, y0, nrows, buf):
         a = np.ascontiguousarray(self.fld[field][:, :, y0:y0 + nrows, :])
-        buf.copy_(torch.from_numpy(a.view(np.uint8).reshape(-1)))
+        buf[:a.nbytes].copy_(torch.from_numpy(a.view(np.uint8).reshape(-1)))
 
     def set_rows(self, field, y0, nrows, buf):
-        a = buf.numpy().view(np.uint64).reshape(COMPS[field], self.shape[0], nrows, self.shape[2])
+        a = buf[:self.rows_bytes(field, nrows)].numpy().view(np.uint64).reshape(COMPS[field], self.shape[0], nrows, self.shape[2])
         self.fld[field][:, :, y0:y0 + nrows, :] = a
+
+    def get_rows_pair(self, field, y0_a, y0_b, nrows, buf):
+        nb = self.rows_bytes(field, nrows)
+        self.get_rows(field, y0_a, nrows, buf[:nb])
+        self.get_rows(field, y0_b, nrows, buf[nb:2 * nb])
+
+    def set_rows_pair(self, field, y0_a, y0_b, nrows, buf):
+        nb = self.rows_bytes(field, nrows)
+        self.set_rows(field, y0_a, nrows, buf[:nb])
+        self.set_rows(field, y0_b, nrows, buf[nb:2 * nb])
 
     def synchronize(self):
         pass

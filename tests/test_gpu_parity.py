@@ -166,6 +166,33 @@ def test_ragged_and_degenerate_grids(shape, gz):
         compare(o, g, *tol, tol_f=None if precision == 0 else 5e-3, label="ragged %s p%d" % (shape, precision))
 
 
+@pytest.mark.parametrize("shape,anchoring,W0", [((64, 8, 5), 0, 0.0), ((128, 21, 9), 0, 0.0), ((192, 7, 12), 1, 2e-3),
+                                                ((64, 40, 23), 1, -1e-3)])
+def test_director_kernel_forms_agree(shape, anchoring, W0):
+    """Rows that are a multiple of 64 cells take the four-cells-per-thread director kernels in FP32 (nh_fd_vec.cuh):
+    against the oracle, and against the one-cell-per-thread tiled (NH_OPT_FD_NOVEC) and plain (NH_OPT_FD_DIRECT)
+    forms of the same update, with ny not a multiple of the tile height, z-chunks of one plane, free plates and W0."""
+    m = nh()
+    nx, ny, nz = shape
+    d = I.noisy_homeotropic(nx, ny, nz, 0.1)
+    p = dict(nx=nx, ny=ny, nz=nz, tau=0.7, K=0.015, pitch=9.0, xi=0.8, gamma1=1.3, g=(2e-6, -1e-6, 1e-6), fd_ratio=2,
+             anchoring=anchoring, W0=W0, director=d)
+    o, g = pair(p, 1)
+    o.step(40)
+    g.step(40)
+    compare(o, g, FP32_TOL_U, FP32_TOL_N, tol_f=5e-3, label="vec %s" % (shape,))
+    ref = g.get_fields()
+    for opt, knobs in ((m.OPT_FD_NOVEC, {}), (m.OPT_FD_DIRECT, {}), (0, dict(fd_planes=1)), (0, dict(fd_planes=3))):
+        _, h = pair(p, 1, options=opt)
+        h.debug_tune(**knobs)
+        h.step(40)
+        f = h.get_fields()
+        assert rel_linf(f["u"], ref["u"]) < 1e-4 and np.abs(f["n"] - ref["n"]).max() < 2e-5, (shape, opt, knobs)
+        if not opt:                      # the same kernels in other z-chunks: the same arithmetic per cell
+            for k in ref:
+                assert np.array_equal(f[k], ref[k]), (shape, knobs, k)
+
+
 @pytest.mark.parametrize("coupling", [0, 1, 2])
 def test_coupling_switches(coupling):
     p = I.config(0, coupling=coupling, fd_ratio=2)
