@@ -518,6 +518,11 @@ def main():
 
         job()
         ms_job = timed(job)
+        # where the job's time goes (each part timed on its own, same buffers): PCIe copies of FP64 host arrays
+        # (the contract's choice) against the device-resident steps
+        ms_h2d = timed(lambda: lat.set_director(d_pinned))
+        ms_steps = timed(lambda: [lat.step(r) for _ in range(args.steps)])
+        ms_d2h = timed(lambda: lat.get_fields(out=out, which=("u", "n")))
 
         def every():
             for _ in range(3):
@@ -530,6 +535,8 @@ def main():
                "h2d_bytes_per_step": 24 * N / args.steps, "d2h_bytes_per_step": 48 * N / args.steps,
                "what": "one job = nh_set_director(pinned host n) + K steps + nh_get_fields(u, n -> pinned host), "
                        "all inside the timed region; bytes are the job's copies divided by K",
+               "split_ms": {"set_director_h2d": ms_h2d, "steps": ms_steps, "get_fields_d2h": ms_d2h, "job": ms_job,
+                            "h2d_gbs": 24 * N / (ms_h2d * 1e-3) / 1e9, "d2h_gbs": 48 * N / (ms_d2h * 1e-3) / 1e9},
                "copies_every_step": {"value": job_mlups(world, nf, r * 3, ms_every), "unit": "MLUPS",
                                      "h2d_bytes_per_step": 24 * N, "d2h_bytes_per_step": 48 * N}}
 

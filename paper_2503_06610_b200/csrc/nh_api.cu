@@ -106,6 +106,7 @@ struct nh_lattice {
   unsigned long long* wave;   // device counters of the two-step kernel: ticket at [0], strip counters from [8], then the flags
   int* wave_err;              // pinned, device-mapped host word the kernel sets when a wavefront wait timed out
   int* wave_err_dev;          // its device address
+  int* flag_host;             // pinned landing place of `flag` (second word of the same allocation)
   unsigned long long wave_epoch, wave_tickets;
   unsigned long long strip_count[32];   // host mirror of the device's per-strip completion counters
   unsigned* order_dev;             // launch order table of the two-step kernel
@@ -857,7 +858,7 @@ int init_typed(nh_lattice* L) {
   {
     Bracket br(L, KC_OTHER);
     nh::store_director_kernel<T><<<blocks_for(N), BLOCK, 0, L->stream>>>(
-        L->stage, (T*)L->n[0], (T*)L->nP, (T*)L->n[1], L->G);
+        L->stage, (T*)L->n[0], (T*)L->nP, (T*)L->n[1], L->G, nullptr);
   }
   NH_CUDA(cudaGetLastError());
   NH_CUDA(cudaStreamSynchronize(L->stream));
@@ -870,7 +871,7 @@ int set_director_typed(nh_lattice* L) {
   {
     Bracket br(L, KC_OTHER);
     nh::store_director_kernel<T><<<blocks_for(N), BLOCK, 0, L->stream>>>(
-        L->stage, (T*)L->n[L->ncur], (T*)L->nP, (T*)L->n[L->ncur ^ 1], L->G);
+        L->stage, (T*)L->n[L->ncur], (T*)L->nP, (T*)L->n[L->ncur ^ 1], L->G, L->flag);
   }
   for (void* fld : {L->n[0], L->n[1], L->nP}) { const int rc = mirror_plates<T>(L, fld); if (rc) return rc; }
   // reading G9: force from the initial director (the viscous part from the current velocity)
@@ -881,22 +882,18 @@ int set_director_typed(nh_lattice* L) {
 template <typename T, bool SH>
 int get_fields_typed(nh_lattice* L, double* rho, double* u, double* n, double* F) {
   const size_t N = L->G.N;
-  if (rho || u) {
-    // stage = [ux uy uz]; rho goes through the first N doubles in a second pass
-    if (u) {
-      Bracket br(L, KC_OTHER);
-      nh::fields_kernel<T, SH><<<blocks_for(N), BLOCK, 0, L->stream>>>(
-          (const T*)L->f[L->cur], (const T*)L->F, nullptr, L->stage, L->G, lb_const<T>(L));
-      br.end();
-      NH_CUDA(cudaMemcpyAsync(u, L->stage, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
-    }
-    if (rho) {
-      Bracket br(L, KC_OTHER);
-      nh::fields_kernel<T, SH><<<blocks_for(N), BLOCK, 0, L->stream>>>(
-          (const T*)L->f[L->cur], (const T*)L->F, L->stage, nullptr, L->G, lb_const<T>(L));
-      br.end();
-      NH_CUDA(cudaMemcpyAsync(rho, L->stage, N * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
-    }
+  // The FP64 staging buffer holds one 3-vector field at a time; each field is converted by one kernel and leaves by
+  // one copy, the conversion of the next field queued behind the copy of the last (one stream, no host waits until
+  // the end).  rho shares the pass over the populations with u when both are asked for.
+  if (u || rho) {
+    Bracket br(L, KC_OTHER);
+    // stage = [ux uy uz]; rho (N doubles) goes to the `a` buffer, which only lives between a predictor and its corrector
+    double* rho_stage = (rho && u) ? (double*)L->a : L->stage;
+    nh::fields_kernel<T, SH><<<blocks_for(N), BLOCK, 0, L->stream>>>(
+        (const T*)L->f[L->cur], (const T*)L->F, rho ? rho_stage : nullptr, u ? L->stage : nullptr, L->G, lb_const<T>(L));
+    br.end();
+    if (u) NH_CUDA(cudaMemcpyAsync(u, L->stage, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
+    if (rho) NH_CUDA(cudaMemcpyAsync(rho, rho_stage, N * sizeof(double), cudaMemcpyDeviceToHost, L->stream));
   }
   const void* src[2] = {L->n[L->ncur], L->F};
   double* dst[2] = {n, F};
@@ -1090,9 +1087,11 @@ int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_strea
   L->wave = (unsigned long long*)take(wave_words(p) * 8);
   L->wave_epoch = 0; L->wave_tickets = 0; L->order_key = -1; L->resident_blocks = -1;
   L->wave_err = nullptr;
-  e = cudaHostAlloc((void**)&L->wave_err, sizeof(int), cudaHostAllocMapped);
+  e = cudaHostAlloc((void**)&L->wave_err, 2 * sizeof(int), cudaHostAllocMapped);
   if (e != cudaSuccess) { delete L; return cuda_fail(e, "cudaHostAlloc(error word)"); }
   *L->wave_err = 0;
+  L->flag_host = L->wave_err + 1;
+  *L->flag_host = 0;
   e = cudaHostGetDevicePointer((void**)&L->wave_err_dev, L->wave_err, 0);
   if (e != cudaSuccess) { cudaFreeHost(L->wave_err); delete L; return cuda_fail(e, "cudaHostGetDevicePointer(error word)"); }
   for (int i = 0; i < 32; ++i) L->strip_count[i] = 0;
@@ -1120,10 +1119,14 @@ int nh_set_director(nh_lattice* L, const double* n_host) {
     Bracket br(L, KC_OTHER);
     nh::check_director_kernel<<<blocks_for(N), BLOCK, 0, L->stream>>>(L->stage, N, L->flag);
   }
-  int flag = 0;
-  NH_CUDA(cudaMemcpyAsync(&flag, L->flag, sizeof(int), cudaMemcpyDeviceToHost, L->stream));
-  NH_CUDA(cudaStreamSynchronize(L->stream));
-  if (flag) return fail(NH_EINVAL, "zero-length or non-finite director vector");
+  NH_CUDA(cudaMemcpyAsync(L->flag_host, L->flag, sizeof(int), cudaMemcpyDeviceToHost, L->stream));
+  // One synchronisation, at the end: the store kernel looks at the device's flag itself and leaves the director alone
+  // if the input was bad; what follows it (plates, force) then recomputes what is already there, bit for bit.  Only
+  // with Leslie viscosities, where the force also takes the velocity of NOW, must the host know before it goes on.
+  if (viscous(L)) {
+    NH_CUDA(cudaStreamSynchronize(L->stream));
+    if (*L->flag_host) return fail(NH_EINVAL, "zero-length or non-finite director vector");
+  }
   int rc;
   switch (L->p.precision) {
     case NH_FP64_SHIFTED: rc = set_director_typed<double, true>(L); break;
@@ -1134,6 +1137,7 @@ int nh_set_director(nh_lattice* L, const double* n_host) {
   if (rc) return rc;
   NH_CUDA(cudaGetLastError());
   NH_CUDA(cudaStreamSynchronize(L->stream));
+  if (*L->flag_host) return fail(NH_EINVAL, "zero-length or non-finite director vector");
   return NH_OK;
 }
 

@@ -249,12 +249,15 @@ check_director_kernel(const double* __restrict__ in, size_t N, int* __restrict__
 
 // normalise in FP64, overwrite the plates with z_hat, store in the device precision
 // into n, n^P and the corrector's output buffer (so its plates are set too)
+// `bad` (may be null): the flag of check_director_kernel; if it is set nothing is stored (the lattice keeps its
+// director and nh_set_director reports NH_EINVAL), so the host need not wait for the check before it enqueues this
 template <typename T>
 __global__ void __launch_bounds__(256)
 store_director_kernel(const double* __restrict__ in, T* __restrict__ n, T* __restrict__ nP,
-                      T* __restrict__ nnew, Geom G) {
+                      T* __restrict__ nnew, Geom G, const int* __restrict__ bad) {
   const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= G.N) return;
+  if (bad && *bad) return;
   const unsigned zz = (unsigned)(c / G.plane);
   double a = 0.0, b = 0.0, d = 1.0;
   if (zz != 0 && zz != (unsigned)G.nz - 1) {
@@ -284,7 +287,7 @@ __global__ void __launch_bounds__(256) fill_f64_kernel(double* __restrict__ p, d
   if (c < n) p[c] = v;
 }
 
-// device precision -> FP64 staging for nh_get_fields (whole grid, 3 components)
+// device precision -> FP64 staging for nh_get_fields (whole grid, 3 components; `out` may sit in mapped host memory)
 template <typename T>
 __global__ void __launch_bounds__(256)
 widen3_kernel(const T* __restrict__ a, double* __restrict__ out, size_t n3) {

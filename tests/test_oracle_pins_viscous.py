@@ -16,6 +16,9 @@ V4  alpha4' alone on a sinusoidal shear wave u_x = a sin(k z): F_x = -(alpha4'/2
 V5  alpha all zero: the force is the elastic force bit for bit (the default path is untouched)
 V6  Poiseuille flow with alpha4' only: the plateau velocity drops as the total viscosity rises,
     u_max(alpha4') / u_max(0) close to nu / (nu + alpha4'/2)  (Newtonian stress 2 mu D = alpha4 D)
+V7  WHERE the explicit viscous force stops being stable when it is frozen for r LB steps:
+    alpha4' alone on a transverse shear wave; amplification per FD period and its |G| = 1 crossing
+    against the closed form that the scheme's own statements give (below)
 """
 import math
 
@@ -166,3 +169,66 @@ def test_V6_extra_newtonian_viscosity_slows_poiseuille_flow():
     # the FD viscous term sees u = 0 on the plate NODES (one spacing away), the LB wall is half-way:
     # the two agree to a few per cent on 16 fluid layers
     assert abs(ratio / expect - 1.0) < 0.05, (ratio, expect)
+
+
+def frozen_force_model(L, tau, r, a4):
+    """Amplification per FD period of the transverse shear wave u_y = a sin(k x), k = 2 pi / L, under the alpha4'
+    force frozen for r LB steps, from the scheme as the paper states it, and the alpha4' at which it reaches -1:
+      - the force is F = -(alpha4'/2) sin^2(k) u                      (Eq. 12's alpha4' D term with Eq. 13 twice: pin V4)
+        evaluated from the velocity of Eq. 21, u = j + F_old/2        (rho = 1), and then frozen
+      - a shear wave of the LB fluid decays by lam = exp(-nu k^2) per step, nu = (tau - 1/2)/3  (pin P13),
+        and every step adds F to the momentum, half before and half after the step's decay (Guo forcing, Eq. 18)
+    so with c = alpha4' sin^2(k)/2 and B = (1 + lam)/2 (1 - lam^r)/(1 - lam):
+        F_n = -c (j_n + F_{n-1}/2),   j_{n+1} = lam^r j_n + B F_n
+    a 2x2 linear map whose dominant eigenvalue is G; G = -1 at c = (1 + lam^r) / (B + (1 + lam^r)/2).
+    Long waves only (lam is the hydrodynamic decay, right to O(k^2))."""
+    nu, k = (tau - 0.5) / 3.0, 2.0 * math.pi / L
+    lam = math.exp(-nu * k * k)
+    lr = lam ** r
+    B = 0.5 * (1.0 + lam) * (1.0 - lr) / (1.0 - lam)
+    c = a4 * math.sin(k) ** 2 / 2.0
+    tr, det = lr - c * B - c / 2.0, -(c / 2.0) * lr
+    disc = math.sqrt(tr * tr - 4.0 * det)
+    G = max(((tr - disc) / 2.0, (tr + disc) / 2.0), key=abs)
+    a4_crit = 2.0 * (1.0 + lr) / (math.sin(k) ** 2 * (B + (1.0 + lr) / 2.0))
+    return G, a4_crit
+
+
+def oracle_amplification(L, tau, r, a4, periods=6, nz=82):
+    """Ratio of the wave's amplitude at the mid-plane between the last two of `periods` FD updates.  The plates are 40
+    cells from the plane that is read: what they seed (a z-structure with a larger discrete k^2, which goes unstable
+    earlier) spreads by viscous diffusion, sqrt(nu T) < 4 cells here, and does not reach it."""
+    k = 2.0 * math.pi / L
+    x = np.arange(L, dtype=np.float64)
+    u = np.zeros((3, nz, 2, L))
+    u[1] = 1e-6 * np.sin(k * x)[None, None, :]
+    u[:, 0] = 0.0
+    u[:, -1] = 0.0
+    o = Oracle(L, 2, nz, tau=tau, K=0.0, fd_ratio=r, coupling=1, alpha=(0, 0, 0, a4, 0, 0))
+    o.set_velocity(u)
+    amps = []
+    for _ in range(periods):
+        o.step(r)
+        uy = o.get_fields()["u"][1, nz // 2, 0, :]
+        amps.append(2.0 / L * (uy * np.sin(k * x)).sum())
+    return amps[-1] / amps[-2]
+
+
+@pytest.mark.parametrize("L,tau,r", [(16, 0.9, 10), (16, 0.9, 4), (32, 1.0, 20)])
+def test_V7_stability_limit_of_the_frozen_viscous_force(L, tau, r):
+    """With the force frozen over r steps the explicit alpha4' term over-corrects: the wave flips sign every FD update
+    and grows once alpha4' exceeds a limit that FALLS with r (for r -> infinity: alpha4'/2 sin^2 k < nu k^2, the
+    explicit viscosity must stay below the lattice's own).  The oracle crosses |G| = 1 where the closed form says."""
+    _, a4c = frozen_force_model(L, tau, r, 0.0)
+    # no extra viscosity: plain decay of the LB shear wave
+    assert abs(oracle_amplification(L, tau, r, 0.0) / math.exp(-(tau - 0.5) / 3.0 * (2 * math.pi / L) ** 2 * r) - 1.0) < 0.01
+    below, above = oracle_amplification(L, tau, r, 0.92 * a4c), oracle_amplification(L, tau, r, 1.08 * a4c)
+    assert -1.0 < below < 0.0 and above < -1.0, (below, above, a4c)
+    for f, got in ((0.92, below), (1.08, above)):
+        G, _ = frozen_force_model(L, tau, r, f * a4c)
+        assert abs(got / G - 1.0) < 0.04, (f, got, G)
+    # the limit falls with r, towards 2 nu k^2 / sin^2 k
+    assert frozen_force_model(L, tau, 8 * r, 0.0)[1] < a4c
+    k = 2 * math.pi / L
+    lam = math.exp(-(tau - 0.5) / 3.0 * k * k)
+    assert frozen_force_model(L, tau, 10 ** 6, 0.0)[1] == pytest.approx(2.0 * (1.0 - lam) / math.sin(k) ** 2, rel=1e-9)
