@@ -67,6 +67,9 @@ def test_slab_calls_reject_null_handles(lib):
     assert lib.nh_set_rows(None, 0, 0, 1, 256) == -1
     assert lib.nh_update_force(None) == -1
     assert lib.nh_defer_force(None, 1) == -1
+    assert lib.nh_get_rows_pair(None, 0, 0, 4, 1, 256) == -1 and b"null handle" in lib.nh_last_error()
+    assert lib.nh_set_rows_pair(None, 0, 0, 4, 1, 256) == -1
+    assert lib.nh_debug_tune(None, 0, 0) == -1
 
 
 def test_null_and_small_workspace(lib):
