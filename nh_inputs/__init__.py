@@ -97,12 +97,18 @@ def skyrmion_tubes(nx: int, ny: int, nz: int, centres, R: float, envelope: bool 
     Distances use the periodic minimum image in x and y.
     """
     z = np.arange(nz, dtype=np.float64)[:, None, None]
-    y = np.arange(ny, dtype=np.float64)[None, :, None]
-    x = np.arange(nx, dtype=np.float64)[None, None, :]
     s = np.sin(math.pi * z / nz) if envelope else np.ones_like(z)
     n = np.zeros((3, nz, ny, nx))
     n[2] = 1.0
+    w = int(math.ceil(R)) + 1                      # a tube only touches the window |x - xc|, |y - yc| <= R
     for (xc, yc) in centres:
+        if 2 * w + 1 >= nx or 2 * w + 1 >= ny:     # the window would wrap onto itself: whole plane
+            ix, iy = np.arange(nx), np.arange(ny)
+        else:
+            ix = np.arange(int(math.floor(xc)) - w, int(math.floor(xc)) + w + 2) % nx
+            iy = np.arange(int(math.floor(yc)) - w, int(math.floor(yc)) + w + 2) % ny
+        y = iy.astype(np.float64)[None, :, None]
+        x = ix.astype(np.float64)[None, None, :]
         dx = x - xc
         dy = y - yc
         dx = dx - nx * np.round(dx / nx)
@@ -112,7 +118,8 @@ def skyrmion_tubes(nx: int, ny: int, nz: int, centres, R: float, envelope: bool 
         theta = math.pi * (1.0 - r / R) * s
         phi = np.arctan2(dy, dx) + 0.0 * z
         tube = np.stack([-np.sin(theta) * np.sin(phi), np.sin(theta) * np.cos(phi), np.cos(theta)])
-        n = np.where(inside[None], tube, n)
+        sel = np.ix_(np.arange(3), np.arange(nz), iy, ix)
+        n[sel] = np.where(inside[None], tube, n[sel])
     return np.ascontiguousarray(_plates_homeotropic(_normalise(n)))
 
 

@@ -416,6 +416,37 @@ def test_config3_full_size_bench_configuration():
     assert np.abs(np.sqrt((f["n"] ** 2).sum(0)) - 1.0).max() < 1e-14
 
 
+def test_config4_largest_grid_properties():
+    """configs[4] at its largest size (512x512x128, 33.5 M cells, about 7 GB in FP32), far beyond what the oracle is
+    run for: what holds at any size.  The default FP32 path there is the two-step LB kernel over FOUR y-strips; it must
+    equal one LB step per launch bit for bit; mass is conserved, |n| = 1, the plates keep their values, and FP32
+    stays close to the FP64 run of the same GPU path."""
+    m = nh()
+    p = I.config(4, size=(512, 512, 128))
+    d = p.pop("director")
+    p.pop("steps")
+    nf = p["nx"] * p["ny"] * (p["nz"] - 2)
+    out = {}
+    for name, precision, opt in (("two", 1, 0), ("one", 1, m.OPT_LB_ONESTEP), ("f64", 0, 0)):
+        g = m.Lattice(**dict(p, precision=precision))
+        g.set_options(opt)
+        g.set_director(d)
+        g.step(23)                                   # two director updates and an odd tail
+        if name == "two":
+            assert g.kernel_time("lb2")[1] > 0       # the two-step kernel is what ran
+        out[name] = g.get_fields(which=("rho", "u", "n"))
+        g.close()
+    for k in out["two"]:
+        assert np.array_equal(out["two"][k], out["one"][k]), k
+    for name, tol_m, tol_n in (("two", 2e-7, 5e-7), ("f64", 1e-12, 1e-14)):
+        f = out[name]
+        assert abs((f["rho"][1:-1] - 1.0).sum()) / nf < tol_m
+        assert np.abs(np.sqrt((f["n"] ** 2).sum(0)) - 1.0).max() < tol_n
+        assert np.all(f["n"][2, 0] == 1.0) and np.all(f["u"][:, -1] == 0.0)
+    assert rel_linf(out["two"]["u"], out["f64"]["u"]) < FP32_TOL_U
+    assert np.abs(out["two"]["n"] - out["f64"]["n"]).max() < FP32_TOL_N
+
+
 def test_config3_full_length_invariants():
     """configs[3] over its full 20 000 LB steps (far beyond what the oracle is run for): properties
     that hold at any length -- mass conserved, |n| = 1, plates fixed, no wavefront error -- and the

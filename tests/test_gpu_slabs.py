@@ -187,3 +187,48 @@ def test_two_processes_exchange_halos_of_real_lattices(tmp_path):
     for rank, (p, o) in enumerate(zip(procs, outs)):
         assert p.returncode == 0, o
         assert "rank %d slabs ok" % rank in o
+
+
+def test_rows_pair_round_trip_and_validation():
+    """nh_get_rows_pair / nh_set_rows_pair: two row ranges in one launch equal two single calls; bad ranges and
+    unknown tuning keys are refused (NH_EINVAL) and leave the lattice alone."""
+    import torch
+    nh = _lib()
+    p = I.config(1, nx=32, ny=20, nz=7, fd_ratio=2)
+    d = p.pop("director")
+    p.pop("steps")
+    for precision in (nh.FP64_SHIFTED, nh.FP32_SHIFTED):
+        g = nh.Lattice(**dict(p, precision=precision))
+        g.set_director(d)
+        g.step(6)
+        for field in ("populations", "director", "velocity", "force"):
+            nb = g.rows_bytes(field, 3)
+            a, b = g.new_rows_buffer(field, 3), g.new_rows_buffer(field, 3)
+            both = g.new_rows_buffer(field, 6)
+            g.get_rows(field, 2, 3, a)
+            g.get_rows(field, 15, 3, b)
+            g.get_rows_pair(field, 2, 15, 3, both)
+            g.synchronize()
+            assert torch.equal(both[:nb], a) and torch.equal(both[nb:2 * nb], b), field
+        before = g.get_fields()
+        # swap the two row ranges of the director through a pair call and back
+        both = g.new_rows_buffer("director", 6)
+        g.get_rows_pair("director", 2, 15, 3, both)
+        g.set_rows_pair("director", 15, 2, 3, both)
+        mid = g.get_fields(which=("n",))["n"]
+        assert np.array_equal(mid[:, :, 15:18], before["n"][:, :, 2:5]) and np.array_equal(mid[:, :, 2:5], before["n"][:, :, 15:18])
+        g.set_rows_pair("director", 2, 15, 3, both)
+        assert np.array_equal(g.get_fields(which=("n",))["n"], before["n"])
+        for bad in ((18, 2), (2, -1), (2, 18)):
+            with pytest.raises(nh.NhError) as ei:
+                g.get_rows_pair("director", bad[0], bad[1], 3, both)
+            assert ei.value.code == -1
+        with pytest.raises(nh.NhError):
+            nh.load().nh_debug_tune  # the symbol exists
+            nh.binding._check(nh.load().nh_debug_tune(g._h, 99, 1))
+        with pytest.raises(nh.NhError):
+            nh.binding._check(nh.load().nh_debug_tune(g._h, 0, -1))
+        after = g.get_fields()
+        for k in before:
+            assert np.array_equal(before[k], after[k]), k
+        g.close()
