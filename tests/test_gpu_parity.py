@@ -340,7 +340,9 @@ def test_two_step_kernel_is_bit_identical(shape, r):
     variants = [(T, {}), (T | m.OPT_NO_SERPENTINE, {}), (T, dict(lb2_cells=1)), (T, dict(lb2_threads=128)),
                 (T, dict(lb2_lead=1, lb2_ring=3)), (T, dict(lb2_lead=3, lb2_ring=12, lb2_blockorder=1)),
                 (T, dict(lb2_blockorder=1, lb2_cells=1)), (T, dict(lb2_strips=2)),
-                (T, dict(lb2_strips=4, lb2_lead=2, lb2_ring=5)), (T, dict(lb2_strips=8, lb2_blockorder=1))]
+                (T, dict(lb2_strips=4, lb2_lead=2, lb2_ring=5)), (T, dict(lb2_strips=8, lb2_blockorder=1)),
+                # four consecutive cells per thread, 16-byte loads and stores (rows a multiple of 128 cells, FP32)
+                (T, dict(lb2_cells=4)), (T, dict(lb2_cells=4, lb2_threads=128, lb2_strips=2))]
     for precision in (0, 1):
         ref = run(precision, m.OPT_LB_ONESTEP, [43])
         for opt, knobs in variants:
