@@ -113,6 +113,7 @@ struct nh_lattice {
   unsigned order_len;
   long long order_key;             // (D << 32) | nzf the table was built for, -1: none
   int sm_count;
+  double ring_budget_mb;           // what the two-step kernel's ring may take of the L2: 38 % of it (48 of B200's 126 MB, measured)
   int resident_blocks;             // co-resident CTAs of lb_resident_kernel on this device (-1: not asked yet)
   int chain_lb;                    // the last launch of this lattice: 1 lb_step_kernel, 2 lb_wave_kernel, 0 anything else
   int defer_force;                 // nh_defer_force: nh_step leaves F^LC to a later nh_update_force
@@ -305,7 +306,7 @@ void lb2_lead(const nh_lattice* L, const PieceGrid& g, int* D, int* R) {
     // D = 4, R = 8 where eight ring planes stay within 48 MB of the L2; a shorter wavefront (D = 3, R = 6) for
     // larger strip-planes (measured on 320x320x64: 35 600 against 34 800 MLUPS with the 63 MB ring, 32 600 one-step)
     const double plane_mb = 19.0 * (g.YS + 2) * L->G.nx * word_of(L->p.precision) / 1e6;
-    if (8.0 * plane_mb > 48.0) { *D = 3; *R = 6; }
+    if (8.0 * plane_mb > L->ring_budget_mb) { *D = 3; *R = 6; }
   }
   if (*D == 0) *D = 4;
   if (*R == 0) *R = *D + 4;
@@ -329,7 +330,7 @@ bool lb2_usable(const nh_lattice* L) {
   // automatic: only where it was measured to pay: FP32, a strip-plane at least as
   // large as the resident CTAs' work, and a ring that fits the L2 beside the streaming traffic
   const double ring_mb = (double)R * 19.0 * (g.YS + 2) * L->G.nx * word_of(L->p.precision) / 1e6;
-  return word_of(L->p.precision) == 4 && (size_t)g.YS * L->G.nx >= 65536 && ring_mb <= 48.0 && L->G.nz - 2 >= 4 * D;
+  return word_of(L->p.precision) == 4 && (size_t)g.YS * L->G.nx >= 65536 && ring_mb <= L->ring_budget_mb && L->G.nz - 2 >= 4 * D;
 }
 
 // upper bound of the pieces of one strip-plane over all piece shapes (sizes the flag arrays)
@@ -487,7 +488,7 @@ int launch_velocity(nh_lattice* L) {
   return NH_OK;
 }
 
-// z-march geometry of the tiled FD kernels: enough CTAs to fill 148 SMs several times over, but
+// z-march geometry of the tiled FD kernels: enough CTAs to fill the SMs several times over, but
 // chunks long enough that the 2 (director) or 4 (force) extra planes per chunk stay cheap
 struct TileGrid { dim3 grid; int zchunk; };
 TileGrid tile_grid(const nh_lattice* L) {
@@ -495,7 +496,7 @@ TileGrid tile_grid(const nh_lattice* L) {
   const int nzf = L->G.nz - 2;
   int zchunk = L->tune[NH_TUNE_FD_PLANES];                   // tuning override
   if (zchunk == 0) {
-    int want = (6 * 148 + tiles - 1) / tiles;                // chunks wanted
+    int want = (6 * L->sm_count + tiles - 1) / tiles;        // chunks wanted
     int most = (nzf + 7) / 8;                                // chunks of >= 8 planes
     if (want > most) want = most;
     if (want < 1) want = 1;
@@ -840,6 +841,9 @@ int init_typed(nh_lattice* L) {
     int dev = 0;
     NH_CUDA(cudaGetDevice(&dev));
     NH_CUDA(cudaDeviceGetAttribute(&L->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    int l2 = 0;
+    NH_CUDA(cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev));
+    L->ring_budget_mb = 0.38 * (double)l2 / 1e6;
   }
   { const int rc = enable_tile_smem<T>(); if (rc) return rc; }
   NH_CUDA(cudaMemsetAsync(L->a, 0, 3 * N * sizeof(T), L->stream));
