@@ -345,6 +345,10 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    # test hooks (tests/test_gpu_slabs.py runs the N = 2 path on a one-GPU box): all ranks on one device, gloo instead of NCCL
+    backend = os.environ.get("NH_BENCH_BACKEND", "nccl")
+    if "NH_BENCH_DEVICE" in os.environ:
+        local = int(os.environ["NH_BENCH_DEVICE"])
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --impl ours needs a CUDA device (there is no CPU path)")
     torch.cuda.set_device(local)
@@ -352,7 +356,10 @@ def main():
     # graph replay (--graph) cannot capture the legacy default stream
     torch.cuda.set_stream(torch.cuda.Stream())
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(backend)
         if rank == 0:
             sys.stderr.write("bench.py: communicator backend=%s nranks=%d (NCCL_DEBUG=INFO shows its rings and NVLS)\n"
                              % (dist.get_backend(), dist.get_world_size()))

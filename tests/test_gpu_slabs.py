@@ -253,3 +253,27 @@ def test_rows_pair_round_trip_and_validation():
         for k in before:
             assert np.array_equal(before[k], after[k]), k
         g.close()
+
+
+def test_bench_starts_its_own_ranks_and_runs_slabs():
+    """`bench.py --gpus 2` outside torchrun starts two ranks itself and runs ONE lattice of twice the rows in two
+    y-slabs (weak scaling), exchanging halos between the processes.  On this one-GPU box both ranks sit on GPU 0 and
+    talk through gloo (test hooks NH_BENCH_DEVICE / NH_BENCH_BACKEND); with N GPUs the same code runs over NCCL."""
+    import json
+    import os
+    import subprocess
+    import sys
+    _lib()
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, NH_BENCH_DEVICE="0", NH_BENCH_BACKEND="gloo")
+    env.pop("WORLD_SIZE", None)
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--config", "1", "--fd-ratio", "4",
+                        "--steps", "3", "--warmup", "3"], env=env, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stdout + r.stderr
+    lines = [x for x in r.stdout.splitlines() if x.startswith("{")]
+    assert len(lines) == 1, r.stdout                      # rank 0 alone prints
+    j = json.loads(lines[0])
+    assert j["n_gpus"] == 2 and j["scaling"] == "weak" and j["value"] > 0 and j["unit"] == "MLUPS"
+    assert j["config"]["grid"] == [64, 128, 32] and j["config"]["parallelism"].startswith("y-slabs x2")
+    assert j["config"]["exchanges_per_step"] > 0 and j["gpu_launches"] > 0
+    assert "nranks=2" in r.stderr
