@@ -14,7 +14,7 @@ extern "C" {
 #define NH_TUNE_LB2_RING         2   /* two-step LB kernel: ring planes R (>= D + 2)                                */
 #define NH_TUNE_LB2_STRIPS       3   /* two-step LB kernel: number of y-strips (must divide ny; <= 32)              */
 #define NH_TUNE_LB2_CELLS        4   /* two-step LB kernel: cells per thread (1, 2 or 4)                            */
-#define NH_TUNE_LB2_THREADS      5   /* two-step LB kernel: 128-thread CTAs (value 128)                             */
+#define NH_TUNE_LB2_THREADS      5   /* two-step LB kernel: threads per CTA, 64 ... 256 in steps of 32 (where they tile) */
 #define NH_TUNE_LB2_BLOCKORDER   6   /* two-step LB kernel: units in blockIdx order instead of by atomic ticket;
                                         relies on in-order CTA dispatch, which CUDA does not promise: tuning only,
                                         a violated order ends in the wait's timeout (NH_ECUDA), not in a hang       */

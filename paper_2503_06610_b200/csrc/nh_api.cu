@@ -251,14 +251,20 @@ int launch_lb(nh_lattice* L) {
 // Geometry of one strip-plane for U cells per thread: YS lattice rows per strip (+ 2 halo rows in the
 // ring), cut into pieces of NT*U cells; false if this grid does not tile into pieces.
 struct PieceGrid { unsigned YS, nstrips, cps, ppr, rows_per_piece, pieces2; int spr_shift; };
-// Threads per CTA for U cells per thread.  256 (or 128 when forced) where rows of nx cells tile into pieces of
-// 256 U cells; otherwise, for two cells per thread, 32 k threads with k the largest divisor of nx / 64 in 3..7
-// (one piece = k warps side by side in one row: nx = 320 -> 160 threads, 384 -> 192, 448 -> 224, 192 -> 96,
-// 576 -> 96 x 3 pieces per row); 0 if there is none.
+// Threads per CTA for U cells per thread.  Where rows of nx cells tile into pieces of 128 U cells: 128 threads for
+// two cells per thread in FP32 (four warps wait less at the CTA's two barriers than eight: measured 2-5 % on every
+// grid), else 256 where pieces of 256 U cells tile.  Otherwise, for two cells per thread, 32 k
+// threads with k the largest divisor of nx / 64 in 3..7 (one piece = k warps side by side in one row: nx = 320 -> 160
+// threads, 384 -> 192, 448 -> 224, 192 -> 96, 576 -> 96 x 3 pieces per row).  nh_debug_tune can force 64 ... 256.
 int lb2_threads(const nh_lattice* L, int U) {
-  if (L->tune[NH_TUNE_LB2_THREADS] == 128) return 128;
-  const unsigned nx = (unsigned)L->G.nx, pc = 256u * U;
-  if (pc % nx == 0 || nx % pc == 0) return 256;
+  const unsigned nx = (unsigned)L->G.nx;
+  const int forced = L->tune[NH_TUNE_LB2_THREADS];
+  auto tiles = [&](unsigned nt) { const unsigned pc = nt * U; return pc % nx == 0 || nx % pc == 0; };
+  if ((forced == 128 || forced == 256) && tiles((unsigned)forced)) return forced;
+  if (forced == 64 && U == 2 && tiles(64)) return 64;
+  if (U == 2 && nx % 64 == 0 && forced >= 96 && forced <= 224 && forced % 32 == 0 && (nx / 64) % (unsigned)(forced / 32) == 0) return forced;
+  if (U == 2 && word_of(L->p.precision) == 4 && tiles(128)) return 128;
+  if (tiles(256)) return 256;
   if (U != 2 || nx % 64) return 256;          // piece_grid will refuse
   const unsigned n64 = nx / 64;
   for (unsigned k = 7; k >= 3; --k) if (n64 % k == 0) return (int)(32 * k);
@@ -429,6 +435,7 @@ int launch_lb2(nh_lattice* L) {
     case 160: return launch_lb2_u<T, SH, 2, 160>(L);
     case 192: return launch_lb2_u<T, SH, 2, 192>(L);
     case 224: return launch_lb2_u<T, SH, 2, 224>(L);
+    case 64: return launch_lb2_u<T, SH, 2, 64>(L);
     case 128: return two ? launch_lb2_u<T, SH, 2, 128>(L) : launch_lb2_u<T, SH, 1, 128>(L);
     default: return two ? launch_lb2_u<T, SH, 2, 256>(L) : launch_lb2_u<T, SH, 1, 256>(L);
   }

@@ -337,7 +337,7 @@ def test_two_step_kernel_is_bit_identical(shape, r):
         return f
 
     T = m.OPT_LB_TWOSTEP
-    variants = [(T, {}), (T | m.OPT_NO_SERPENTINE, {}), (T, dict(lb2_cells=1)), (T, dict(lb2_threads=128)),
+    variants = [(T, {}), (T | m.OPT_NO_SERPENTINE, {}), (T, dict(lb2_cells=1)), (T, dict(lb2_threads=256)), (T, dict(lb2_threads=64)),
                 (T, dict(lb2_lead=1, lb2_ring=3)), (T, dict(lb2_lead=3, lb2_ring=12, lb2_blockorder=1)),
                 (T, dict(lb2_blockorder=1, lb2_cells=1)), (T, dict(lb2_strips=2)),
                 (T, dict(lb2_strips=4, lb2_lead=2, lb2_ring=5)), (T, dict(lb2_strips=8, lb2_blockorder=1)),
