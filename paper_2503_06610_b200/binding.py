@@ -24,7 +24,8 @@ KERNEL_CLASSES = ("lb", "velocity", "predictor", "corrector", "force", "other", 
 EXPORTS = ("nh_workspace_bytes", "nh_init_lattice", "nh_set_director", "nh_step", "nh_get_fields",
            "nh_time", "nh_launch_count", "nh_set_options", "nh_kernel_time", "nh_free", "nh_last_error",
            "nh_rows_bytes", "nh_get_rows", "nh_set_rows", "nh_update_force", "nh_defer_force", "nh_debug_tune",
-           "nh_get_rows_pair", "nh_set_rows_pair")
+           "nh_get_rows_pair", "nh_set_rows_pair", "nh_lb_two_steps_noalloc")
+NOALLOC_SCRATCH_BYTES = 16 * 1024 * 1024      # NH_NOALLOC_SCRATCH_BYTES of include/nh_noalloc.h
 
 
 class NhParams(C.Structure):
@@ -79,6 +80,8 @@ def load():
         lib.nh_update_force.argtypes = [C.c_void_p]
         lib.nh_defer_force.argtypes = [C.c_void_p, C.c_int]
         lib.nh_debug_tune.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        lib.nh_lb_two_steps_noalloc.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_double),
+                                                C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.nh_free.argtypes = [C.c_void_p]
         lib.nh_free.restype = None
         lib.nh_last_error.restype = C.c_char_p
@@ -112,6 +115,20 @@ def _host_ptr(a):
     assert isinstance(a, torch.Tensor) and a.device.type == "cpu" and a.dtype == torch.float64
     assert a.is_contiguous()
     return a.data_ptr()
+
+
+def lb_two_steps_noalloc(nx, ny, nz, precision, tau, g, f_in, F_lc, f_out, stream=None):
+    """nh_lb_two_steps_noalloc (include/nh_noalloc.h): f_out := two LB steps of f_in, for callers that may not allocate
+    device memory -- the kernel's ring and flags sit in an array inside the library, nothing is allocated here or there.
+    f_in, f_out: CUDA tensors holding [19][nz][ny][nx] words of the precision's type; F_lc: [3][nz][ny][nx] or None.
+    All on the current device; `stream` a torch stream of that device (default: the current one).  Returns when done."""
+    import torch
+    for t in (f_in, f_out) + ((F_lc,) if F_lc is not None else ()):
+        assert t.is_cuda and t.is_contiguous()
+    s = stream if stream is not None else torch.cuda.current_stream(f_in.device)
+    _check(load().nh_lb_two_steps_noalloc(int(nx), int(ny), int(nz), int(precision), float(tau), (C.c_double * 3)(*g),
+                                          f_in.data_ptr(), F_lc.data_ptr() if F_lc is not None else None,
+                                          f_out.data_ptr(), s.cuda_stream))
 
 
 class Lattice:

@@ -4,6 +4,7 @@
 // kernels of nh_lb.cuh / nh_fd.cuh.
 #include "../../include/nh.h"
 #include "../../include/nh_debug.h"
+#include "nh_internal.h"
 
 #include <cuda_runtime.h>
 
@@ -1037,6 +1038,9 @@ int rows_check(nh_lattice* L, int y0, int nrows, const void* buf) {
 bool is_f32(const nh_lattice* L) { return L->p.precision == NH_FP32_SHIFTED || L->p.precision == NH_FP32_UNSHIFTED; }
 
 }  // namespace
+
+// the other translation units report through the same per-thread text (nh_internal.h)
+int nh::set_error(int code, const char* msg) { return fail(code, msg); }
 
 extern "C" {
 

@@ -20,7 +20,7 @@ def lib():
 
 def declared_symbols():
     names = set()
-    for header in sorted(os.listdir(os.path.join(ROOT, "include"))):      # nh.h (the contract), nh_debug.h (hooks)
+    for header in sorted(os.listdir(os.path.join(ROOT, "include"))):      # nh.h (the contract), nh_debug.h (hooks), nh_noalloc.h
         text = open(os.path.join(ROOT, "include", header)).read()
         text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
         names |= set(re.findall(r"\b(nh_[a-z_]+)\s*\(", text))
@@ -113,3 +113,25 @@ def test_product_does_not_import_the_oracle():
             src = open(os.path.join(ROOT, "oracle", fn)).read()
             assert "paper_2503_06610_b200 import" not in src and "import paper_2503_06610_b200" not in src, fn
             assert "nh_lb.cuh" not in src and "include/nh.h" not in src, fn
+
+
+def test_no_alloc_entry_validates_before_it_touches_cuda(lib):
+    """nh_lb_two_steps_noalloc (include/nh_noalloc.h): bad arguments and lattices beyond the 16 MiB static scratch are
+    refused with NH_EINVAL before any CUDA call; with good arguments and no device it is NH_ECUDA (no CPU path)."""
+    g = (C.c_double * 3)(0.0, 0.0, 0.0)
+    call = lambda nx, ny, nz, prec, tau, a=4096, b=1 << 40: lib.nh_lb_two_steps_noalloc(nx, ny, nz, prec, tau, g, a, None, b, None)
+    assert call(512, 512, 64, 1, 0.8) == -1 and b"beyond the static scratch" in lib.nh_last_error()
+    assert call(256, 256, 16, 0, 0.8) == -1 and b"16777216" in lib.nh_last_error()
+    assert call(96, 8, 6, 1, 0.8) == -1 and b"nx must be" in lib.nh_last_error()
+    assert call(64, 8, 4, 1, 0.8) == -1
+    assert call(64, 8, 6, 1, 0.5) == -1
+    assert call(64, 8, 6, 9, 0.8) == -1
+    assert call(64, 8, 6, 1, 0.8, a=4096, b=4096) == -1 and b"overlap" in lib.nh_last_error()
+    assert lib.nh_lb_two_steps_noalloc(64, 8, 6, 1, 0.8, None, 4096, None, 1 << 40, None) == -1
+    try:
+        import torch
+        has_gpu = torch.cuda.is_available()
+    except Exception:
+        has_gpu = False
+    if not has_gpu:
+        assert call(64, 8, 6, 1, 0.8) == -3 and lib.nh_last_error()
