@@ -118,6 +118,9 @@ struct nh_lattice {
   int resident_blocks;             // co-resident CTAs of lb_resident_kernel on this device (-1: not asked yet)
   int chain_lb;                    // the last launch of this lattice: 1 lb_step_kernel, 2 lb_wave_kernel, 0 anything else
   int defer_force;                 // nh_defer_force: nh_step leaves F^LC to a later nh_update_force
+  int vec_grid_known[2];           // launch shape of director_vec_kernel<., STAGE>, worked out at its first launch
+  dim3 vec_grid_dim[2];
+  int vec_grid_zchunk[2];
   // CUDA-graph replay of nh_step (NH_OPT_GRAPH): one executable graph per distinct call shape
   struct Graph {
     int n_lb, r, phase, cur, ncur, sweep, options;   // key: arguments and the state the launches depend on
@@ -526,8 +529,9 @@ bool tiles_fit(const nh_lattice* L) {
 // ---- four cells per thread along x (nh_fd_vec.cuh): FP32, rows a multiple of 64 cells ----------------------
 template <typename T>
 bool vec_usable(const nh_lattice* L) {
+  // (the kernel and its stager keep element offsets comp * N + cell in 32 bits)
   return sizeof(T) == 4 && L->G.nx % nh::VW == 0 && !(L->options & (NH_OPT_FD_DIRECT | NH_OPT_FD_NOVEC)) &&
-         (L->G.ny + nh::VTY - 1) / nh::VTY <= 65535;
+         (L->G.ny + nh::VTY - 1) / nh::VTY <= 65535 && 3.0 * (double)L->G.N < 4294967296.0;
 }
 // z-chunks of the march: the number of chunks per tile that minimises (waves of CTAs) x (planes per chunk + the
 // `prime` planes a chunk stages before its first result), with `per_sm` CTAs resident per SM
@@ -555,9 +559,15 @@ int launch_director_vec(nh_lattice* L, const nh::FdConst<T>& C, int with_flow, c
   Bracket br(L, cls);
   if (br.rc) return br.rc;
   const size_t sm = nh::director_vec_smem_bytes<T>();
-  int per_sm = 0;
-  NH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, nh::director_vec_kernel<T, STAGE>, nh::VTHREADS, sm));
-  const TileGrid g = vec_grid(L, per_sm, 2);
+  // occupancy and the z-chunk search once per lattice and stage (nh_debug_tune forgets them)
+  if (!L->vec_grid_known[STAGE]) {
+    int per_sm = 0;
+    NH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, nh::director_vec_kernel<T, STAGE>, nh::VTHREADS, sm));
+    const TileGrid fresh = vec_grid(L, per_sm, 2);
+    L->vec_grid_dim[STAGE] = fresh.grid; L->vec_grid_zchunk[STAGE] = fresh.zchunk; L->vec_grid_known[STAGE] = 1;
+  }
+  TileGrid g;
+  g.grid = L->vec_grid_dim[STAGE]; g.zchunk = L->vec_grid_zchunk[STAGE];
   nh::director_vec_kernel<T, STAGE><<<g.grid, nh::VTHREADS, sm, L->stream>>>(field, (const T*)L->u, a_in, out, a_out, L->G, C,
                                                                             with_flow, g.zchunk);
   br.end();
@@ -1020,6 +1030,7 @@ int rows_typed(nh_lattice* L, int field, int y0a, int y0b, int ranges, int nrows
   if (rc) return rc;
   const size_t half = (size_t)comps * L->G.nz * nrows * L->G.nx, total = half * ranges;
   if (total == 0) return NH_OK;
+  if (total >= 4294967296ull) return fail(NH_EINVAL, "too many rows for one call: the packed buffer must stay below 2^32 words");
   Bracket br(L, KC_OTHER);
   rows_kernel<T, PACK><<<blocks_for(total), BLOCK, 0, L->stream>>>((T*)base, (T*)buf, L->G, y0a, y0b, nrows, (unsigned)half, (unsigned)total);
   br.end();
@@ -1137,8 +1148,10 @@ int nh_set_director(nh_lattice* L, const double* n_host) {
   NH_CUDA(cudaMemcpyAsync(L->flag_host, L->flag, sizeof(int), cudaMemcpyDeviceToHost, L->stream));
   // One synchronisation, at the end: the store kernel looks at the device's flag itself and leaves the director alone
   // if the input was bad; what follows it (plates, force) then recomputes what is already there, bit for bit.  Only
-  // with Leslie viscosities, where the force also takes the velocity of NOW, must the host know before it goes on.
-  if (viscous(L)) {
+  // with Leslie viscosities, where the force also takes the velocity of NOW, must the host know before it goes on --
+  // and under nh_defer_force, where F^LC may hold halo rows that came from a neighbour (nh_set_rows) and that a local
+  // recomputation would overwrite with values of this slab's periodic wrap.
+  if (viscous(L) || L->defer_force) {
     NH_CUDA(cudaStreamSynchronize(L->stream));
     if (*L->flag_host) return fail(NH_EINVAL, "zero-length or non-finite director vector");
   }
@@ -1239,6 +1252,7 @@ int nh_debug_tune(nh_lattice* L, int key, int value) {
     L->graphs.clear();
   }
   L->tune[key] = value;
+  L->vec_grid_known[0] = L->vec_grid_known[1] = 0;
   return NH_OK;
 }
 
@@ -1247,8 +1261,19 @@ long nh_launch_count(const nh_lattice* L) { return L ? L->launches : -1; }
 
 int nh_set_options(nh_lattice* L, int options) {
   if (!L) return fail(NH_EINVAL, "null handle");
+  constexpr int known = NH_OPT_GRAPH | NH_OPT_TIMING | NH_OPT_FD_DIRECT | NH_OPT_NO_SERPENTINE | NH_OPT_FD_NOVEC |
+                        NH_OPT_LB_TWOSTEP | NH_OPT_LB_ONESTEP;
+  if (options & ~known) return fail(NH_EINVAL, "unknown option bit (launch-shape knobs moved to nh_debug_tune, include/nh_debug.h)");
   int rc = drain_events(L);
   if (rc) return rc;
+  // captured graphs carry the kernels the old bits chose (their key holds the options, so they would never be replayed
+  // wrongly, only kept for nothing): drop them when a kernel-selecting bit changes
+  constexpr int selects = NH_OPT_FD_DIRECT | NH_OPT_NO_SERPENTINE | NH_OPT_FD_NOVEC | NH_OPT_LB_TWOSTEP | NH_OPT_LB_ONESTEP;
+  if (((options ^ L->options) & selects) && !L->graphs.empty()) {
+    NH_CUDA(cudaStreamSynchronize(L->stream));
+    for (auto& g : L->graphs) cudaGraphExecDestroy(g.exec);
+    L->graphs.clear();
+  }
   L->options = options;
   for (int k = 0; k < KC_COUNT; ++k) { L->ms[k] = 0.0; L->cnt[k] = 0; }
   return NH_OK;

@@ -310,6 +310,43 @@ def test_options_do_not_change_results():
         assert g.launch_count > 81
 
 
+def test_unknown_option_bits_are_refused_and_option_changes_drop_graphs():
+    """nh_set_options: bits that are not in include/nh.h (the launch-shape bits of earlier builds, now nh_debug_tune
+    keys) are NH_EINVAL and leave the options as they were; switching a kernel-selecting bit while graphs are held
+    drops them, and the steps that follow are those of a lattice that ran with plain launches throughout."""
+    import torch
+    m = nh()
+    p = I.config(0, fd_ratio=3)
+    d = p.pop("director")
+    p.pop("steps")
+    g = m.Lattice(stream=torch.cuda.Stream(), **dict(p, precision=0))
+    g.set_options(m.OPT_GRAPH)
+    for bad in (8, 1 << 26, 1 << 8, m.OPT_GRAPH | (1 << 30)):
+        with pytest.raises(m.NhError) as ei:
+            g.set_options(bad)
+        assert ei.value.code == -1 and "unknown option bit" in str(ei.value)
+    g.set_director(d)
+    for _ in range(4):
+        g.step(6)                                   # captured once, replayed three times
+    g.set_options(m.OPT_GRAPH | m.OPT_FD_DIRECT)    # other FD kernels: the held graphs go
+    for _ in range(4):
+        g.step(6)
+    g.set_options(m.OPT_GRAPH)
+    g.step(6)
+    h = m.Lattice(**dict(p, precision=0))
+    h.set_director(d)
+    h.step(24)
+    h.set_options(m.OPT_FD_DIRECT)
+    h.step(24)
+    h.set_options(0)
+    h.step(6)
+    fg, fh = g.get_fields(), h.get_fields()
+    for k in fg:
+        assert np.array_equal(fg[k], fh[k]), k
+    assert g.time == h.time == 54
+
+
+
 @pytest.mark.parametrize("shape,r", [((64, 64, 32), 10), ((128, 5, 20), 7), ((32, 7, 9), 3), ((512, 4, 6), 2),
                                      ((1024, 3, 5), 2), ((64, 3, 3), 2), ((256, 9, 8), 4), ((16, 16, 8), 1),
                                      ((128, 24, 12), 3), ((512, 16, 9), 4), ((64, 40, 7), 2),

@@ -255,6 +255,39 @@ def test_rows_pair_round_trip_and_validation():
         g.close()
 
 
+def test_rejected_director_leaves_a_deferred_force_alone():
+    """Under nh_defer_force the force field may hold halo rows that a neighbour sent (nh_set_rows) and that differ from
+    what this lattice would compute from its own periodic wrap.  A director that nh_set_director refuses must leave
+    every field, F^LC included, bit for bit as it was."""
+    nh = _lib()
+    p = I.config(1, nx=32, ny=20, nz=7, fd_ratio=2)
+    d = p.pop("director")
+    p.pop("steps")
+    for precision in (nh.FP64_SHIFTED, nh.FP32_SHIFTED):
+        g = nh.Lattice(**dict(p, precision=precision))
+        g.set_director(d)
+        g.step(4)
+        g.defer_force(True)
+        # rows 0..2 of F take the values of rows 9..11: not what the local stencil gives there
+        own = g.get_fields(which=("F",))["F"]
+        assert not np.array_equal(own[:, 1:-1, 0:3], own[:, 1:-1, 9:12])
+        rows = g.new_rows_buffer("force", 3)
+        g.get_rows("force", 9, 3, rows)
+        g.set_rows("force", 0, 3, rows)
+        before = g.get_fields()
+        bad = d.copy()
+        bad[:, 2, 3, 4] = 0.0
+        with pytest.raises(nh.NhError) as ei:
+            g.set_director(bad)
+        assert ei.value.code == -1
+        after = g.get_fields()
+        for k in before:
+            assert np.array_equal(before[k], after[k]), (precision, k)
+        # and the rows are still the neighbour's, not a local recomputation
+        assert np.array_equal(after["F"][:, 1:-1, 0:3], after["F"][:, 1:-1, 9:12])
+        g.close()
+
+
 def test_bench_starts_its_own_ranks_and_runs_slabs():
     """`bench.py --gpus 2` outside torchrun starts two ranks itself and runs ONE lattice of twice the rows in two
     y-slabs (weak scaling), exchanging halos between the processes.  On this one-GPU box both ranks sit on GPU 0 and
