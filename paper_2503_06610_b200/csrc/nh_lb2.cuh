@@ -119,7 +119,11 @@ __device__ __forceinline__ bool deps_ready(const Wave& W, int phase, int k, unsi
     // the slot was last used by the previous strip: all of it must be done
     ok = ld_acquire_u64(W.strip_done + (strip - 1)) >= W.strip_target[strip - 1];
   }
-  return __all_sync(0xffffffffu, ok);
+  const bool all = __all_sync(0xffffffffu, ok);
+  // The vote carries no memory ordering of its own, and the lanes that go on to read the ring are not only the ones
+  // that did the acquire loads: the warp barrier orders every lane's later loads after all of those acquires.
+  __syncwarp();
+  return all;
 }
 
 // f_i(x, t) = f*_i(x - e_i, t-1) with half-way bounce-back for the U cells (xA + 32 j, y) of one
