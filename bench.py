@@ -98,6 +98,35 @@ def workload(args):
     return p, d, desc
 
 
+B200_L2_MB = 126.0          # nominal L2 of a B200: the config line's L2 statement depends on the workload only, so
+                            # that both arms (--impl ours / reference) print the same `config`
+
+
+def base_options(args):
+    # NH_OPT_LB_TWOSTEP, NH_OPT_LB_ONESTEP, NH_OPT_GRAPH of include/nh.h (literal: the reference arm prints the same
+    # config and must not import the CUDA package)
+    return args.options | (64 if args.two_step else 0) | (128 if args.one_step else 0) | (1 if args.graph else 0)
+
+
+def tune_knobs(args):
+    return {kv.split("=")[0]: int(kv.split("=")[1]) for kv in args.tune}
+
+
+def config_of(args, p, desc, world):
+    """The `config` of the JSON line: the workload and how a step is counted.  The same for both arms."""
+    r = max(1, p["fd_ratio"])
+    N = p["nx"] * p["ny"] * p["nz"]
+    word = 8 if PRECISIONS[args.precision] in (0, 3) else 4
+    pop_mb = 19 * N * word / 1e6
+    fits = 2 * pop_mb <= B200_L2_MB * 1.048576
+    l2 = (("populations (2 x %.0f MB) exceed the %.0f MB L2; no flush needed" if not fits else
+           "populations (2 x %.1f MB) FIT the %.0f MB L2 and nothing is flushed between steps: this grid is "
+           "L2-resident by nature (a time step follows a time step); MLUPS is the figure, GB/s is not") % (pop_mb, B200_L2_MB))
+    return dict(desc, lb_steps_per_step=r, fluid_cells=p["nx"] * p["ny"] * (p["nz"] - 2),
+                step="one step = %d LB steps + 1 director update + 1 force update" % r,
+                parallelism="replicas x%d" % world, l2=l2, options=base_options(args), tune=tune_knobs(args))
+
+
 def peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -195,7 +224,7 @@ class ClockSampler:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
         sm.sort()
         return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons),
-                "samples": len(sm), "power_w_max": max(power)}
+                "samples": len(sm), "power_w_max": max(power), "power_w_mean": sum(power) / len(power)}
 
 
 def run_reference(args):
@@ -208,17 +237,21 @@ def run_reference(args):
     o = Oracle(**dict(p, precision=PRECISIONS[args.precision]))
     o.set_director(d)
     nf = p["nx"] * p["ny"] * (p["nz"] - 2)
-    o.step(args.warmup)
+    r = max(1, p["fd_ratio"])
+    # a step is what the GPU arm calls a step: r LB steps, then the director and force update (one FD period)
+    for _ in range(args.warmup):
+        o.step(r)
     t0 = time.perf_counter()
-    o.step(args.steps)
+    for _ in range(args.steps):
+        o.step(r)
     dt = time.perf_counter() - t0
-    mlups = nf * args.steps / dt / 1e6
-    sample = ("each step = one LB step of the full grid, the FD update firing on every %d-th "
-              "(%d steps timed)" % (p["fd_ratio"], args.steps))
+    mlups = nf * r * args.steps / dt / 1e6
+    sample = ("each step = %d LB steps + 1 FD update of the full %dx%dx%d grid (%d steps timed, %.1f s)"
+              % (r, p["nx"], p["ny"], p["nz"], args.steps, dt))
     line = {"impl": "reference", "metric": METRIC, "value": mlups, "unit": "MLUPS", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": desc,
+            "data": "synthetic", "config": config_of(args, p, desc, 1),
             "cpu_baseline": {"value": mlups, "unit": "MLUPS", "cores": num_threads(), "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": mlups, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -283,6 +316,11 @@ def run_slabs(args, world, rank, local):
     lat = SlabLattice(slabs=nslabs, group=dist.group.WORLD if world > 1 else None, device="cuda:%d" % local,
                       **dict(p, precision=prec))
     lat.set_director(d)
+    # the kernel-variant flags act on every slab's lattice, as they do on the undivided one
+    base_opt, knobs = base_options(args), tune_knobs(args)
+    for L in lat.local.values():
+        L.debug_tune(**knobs)
+        L.set_options(base_opt)
 
     def barrier():
         torch.cuda.synchronize()
@@ -307,6 +345,15 @@ def run_slabs(args, world, rank, local):
     ms = max_over_ranks(ev0.elapsed_time(ev1), world)
     launches = sum(x.launch_count for x in lat.local.values()) - l0
     clocks = sampler.stop() if rank == 0 else None
+    # second pass of the same steps with an event pair around every launch: where each slab's time goes
+    for L in lat.local.values():
+        L.set_options((base_opt & ~nh.OPT_GRAPH) | nh.OPT_TIMING)
+    barrier()
+    for _ in range(args.steps):
+        lat.step(r)
+    kernel_ms = {str(sl): {k: round(L.kernel_time(k)[0], 4) for k in nh.KERNEL_CLASSES} for sl, L in sorted(lat.local.items())}
+    for L in lat.local.values():
+        L.set_options(base_opt)
     if rank == 0:
         line = {"metric": METRIC, "value": nf * r * args.steps / (ms * 1e-3) / 1e6, "unit": "MLUPS", "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -314,8 +361,11 @@ def run_slabs(args, world, rank, local):
                 "config": dict(desc, grid=[p["nx"], p["ny"], p["nz"]], lb_steps_per_step=r, fluid_cells=nf,
                                parallelism="y-slabs x%d, halo %d rows%s" % (nslabs, lat.H, "" if world > 1 else " (one device)"),
                                exchanges_per_step=(lat.exchanges - x0) / args.steps,
-                               halo_bytes_sent_per_step_per_process=(lat.bytes_sent - b0) / args.steps),
-                "clocks": clocks, "gpu_launches": launches, "roofline": None}
+                               halo_bytes_sent_per_step_per_process=(lat.bytes_sent - b0) / args.steps,
+                               options=base_opt, tune=knobs),
+                "clocks": clocks, "gpu_launches": launches, "roofline": None,
+                "kernel_ms_per_slab": {"slabs_of_rank_0": kernel_ms,
+                                       "timed": "second pass of the same K steps with per-launch CUDA events"}}
         print(json.dumps(line))
     if world > 1:
         dist.barrier()
@@ -381,9 +431,8 @@ def main():
     lat = nh.Lattice(device="cuda:%d" % local, **dict(p, precision=prec))
     d_pinned = torch.from_numpy(d).pin_memory()
     lat.set_director(d_pinned)
-    base_opt = (args.options | (nh.OPT_LB_TWOSTEP if args.two_step else 0) | (nh.OPT_LB_ONESTEP if args.one_step else 0)
-                | (nh.OPT_GRAPH if args.graph else 0))
-    knobs = {kv.split("=")[0]: int(kv.split("=")[1]) for kv in args.tune}
+    base_opt = base_options(args)
+    knobs = tune_knobs(args)
     lat.debug_tune(**knobs)
     l2_bytes = int(getattr(torch.cuda.get_device_properties(local), "L2_cache_size", 0)) or 126 * 1024 * 1024
     peak, peak_src = peaks()
@@ -438,7 +487,11 @@ def main():
         traffic, inst, tsrc = ncu_traffic(precision_name + ("+2step" if two else ""), desc["grid"])
         pop_bytes = 2 * 19 * N * w
         in_l2 = pop_bytes <= l2_bytes
-        roof = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak,
+        # The one-step kernels move their algorithmic bytes through the DRAM at the copy rate: HBM-bound.  The two-step
+        # kernel halves the DRAM traffic through the L2 and is then held by latency (barrier and scoreboard stalls,
+        # DRAM and L2 each about half busy: profiles/r02_lbwave_full.txt), so `frac` against the section-8(d) byte model
+        # exceeds 1 and the fraction that says how far it is from ITS limit is own_dram_floor_frac below.
+        roof = {"bound": "latency" if two else "hbm", "kernel": kname, "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": tsrc,
                 "peak_source": peak_src, "frac_of_nominal_8000_gbs": achieved / 8000.0,
                 "algorithmic_bytes_per_launch": alg_bytes,
@@ -463,6 +516,13 @@ def main():
             sms = torch.cuda.get_device_properties(local).multi_processor_count
             roof["issue_frac"] = inst / (lb_avg * 1e-3) / (sms * 4 * clocks["sm_mhz"] * 1e6)
             roof["warp_instructions_per_launch"] = inst
+        if two and lb_avg > 0:
+            # the kernel's own DRAM floor: 19 read + 19 written + 3 (F^LC) words per cell for the PAIR of steps
+            roof["own_dram_floor_bytes_per_launch"] = 41 * w * nf
+            roof["own_dram_floor_frac"] = 41 * w * nf / (lb_avg * 1e-3) / 1e9 / peak
+            roof["bound_is"] = ("latency: two LB steps per pass over HBM through an L2-resident plane ring; neither DRAM "
+                                "nor L2 nor the issue slots are saturated (profiles/): own_dram_floor_frac = time at the "
+                                "measured copy rate for the kernel's own 41 words per cell and launch / measured time")
         if two:
             roof["note"] = ("two LB steps share one pass over HBM (the intermediate step lives in an L2-resident "
                             "plane ring), so the algorithmic bytes of two steps move in about the DRAM traffic of "
@@ -487,6 +547,15 @@ def main():
                      "seconds": ms_long * 1e-3, "ms_per_step": ms_long / reps, "clocks": cl,
                      "what": "the headline loop (same lattice, same options) repeated back to back for at least 3 s, "
                              "clocks and throttle reasons sampled over that window"}
+        if cl and cl.get("power_w_mean"):
+            sustained["mlups_per_watt"] = sustained["value"] / cl["power_w_mean"]
+        # the issue-slot ceiling at the clock the SMs run at under load (the headline's few samples are mostly idle ones)
+        inst = roofline.get("warp_instructions_per_launch")
+        if inst and cl and cl.get("sm_mhz") and roofline["avg_launch_ms"] > 0:
+            sms = torch.cuda.get_device_properties(local).multi_processor_count
+            roofline["issue_frac"] = inst / (roofline["avg_launch_ms"] * 1e-3) / (sms * 4 * cl["sm_mhz"] * 1e6)
+            roofline["issue_frac_clock_mhz"] = cl["sm_mhz"]
+            roofline["issue_frac_clock_from"] = "sustained window"
 
     # ---- what `metric` also names: FP64, and the one-step FP32 kernel, each timed like the headline ----
     extras = {}
@@ -556,13 +625,7 @@ def main():
     line = {"metric": METRIC, "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": DTYPE[prec], "data": "synthetic",
-            "config": dict(desc, lb_steps_per_step=r, fluid_cells=nf, parallelism="replicas x%d" % world,
-                           l2=(("populations (2 x %.0f MB) exceed the %.0f MB L2; no flush needed"
-                                if not m["in_l2"] else
-                                "populations (2 x %.1f MB) FIT the %.0f MB L2 and nothing is flushed between steps: this grid is "
-                                "L2-resident by nature (a time step follows a time step); MLUPS is the figure, GB/s is not")
-                               % (19 * N * word / 1e6, l2_bytes / 1e6)),
-                           options=base_opt, tune=knobs),
+            "config": config_of(args, p, desc, world),
             "clocks": clocks, "gpu_launches": launches, "roofline": roofline}
     if sustained is not None:
         line["sustained"] = sustained

@@ -42,7 +42,7 @@ int cuda_fail(cudaError_t e, const char* what) {
   return nh::set_error(NH_ECUDA, msg);
 }
 int bad(const char* why) {
-  char msg[256];
+  char msg[320];
   std::snprintf(msg, sizeof msg, "nh_lb_two_steps_noalloc: %s", why);
   return nh::set_error(NH_EINVAL, msg);
 }

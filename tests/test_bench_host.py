@@ -50,7 +50,7 @@ def test_single_rank_aggregation_is_identity():
 
 def test_reference_arm_rank_handling():
     """--impl reference: rank 0 alone runs the oracle and prints the line; other ranks exit 0 silently."""
-    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "0",
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "0", "--fd-ratio", "4",
            "--steps", "20", "--warmup", "3", "--gpus", "2"]
     r1 = subprocess.run(cmd, env=dict(os.environ, RANK="1", WORLD_SIZE="2"), capture_output=True, text=True, timeout=600)
     assert r1.returncode == 0 and r1.stdout.strip() == ""
@@ -61,3 +61,23 @@ def test_reference_arm_rank_handling():
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
     assert line["steps"] == 20 and line["warmup"] == 3 and line["n_gpus"] == 2
+    # a step is counted as the GPU arm counts it (r LB steps + one director and force update), and the config dict is
+    # the one the GPU arm prints for the same command line
+    sys.path.insert(0, ROOT)
+    import bench
+    sys.argv, keep = ["bench.py"] + cmd[2:], sys.argv
+    try:
+        args = bench.parse()
+    finally:
+        sys.argv = keep
+    p, d, desc = bench.workload(args)
+    assert line["config"] == json.loads(json.dumps(bench.config_of(args, p, desc, 1)))
+    assert line["config"]["lb_steps_per_step"] == 4 and "4 LB steps" in line["config"]["step"]
+    nf = 16 * 16 * 6
+    assert line["value"] == pytest.approx(nf * 4 / (line["ms_per_step"] * 1e-3) / 1e6, rel=1e-6)
+
+
+def test_bench_source_has_one_config_builder():
+    """Both arms take `config` from bench.config_of, so the driver's same_config comparison holds by construction."""
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert src.count('"config": config_of(') == 2

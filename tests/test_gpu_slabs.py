@@ -310,3 +310,13 @@ def test_bench_starts_its_own_ranks_and_runs_slabs():
     assert j["config"]["grid"] == [64, 128, 32] and j["config"]["parallelism"].startswith("y-slabs x2")
     assert j["config"]["exchanges_per_step"] > 0 and j["gpu_launches"] > 0
     assert "nranks=2" in r.stderr
+    per_slab = j["kernel_ms_per_slab"]["slabs_of_rank_0"]
+    assert len(per_slab) == 1 and all(v["lb"] + v["lb2"] > 0 and v["force"] > 0 for v in per_slab.values())
+    # kernel-variant flags reach the slabs' lattices: --two-step forces two-step launches on a grid that would not take them
+    r1 = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--slabs", "2", "--config", "1", "--fd-ratio", "4",
+                         "--two-step", "--steps", "3", "--warmup", "3"], env=env, capture_output=True, text=True, timeout=900)
+    assert r1.returncode == 0, r1.stdout + r1.stderr
+    j1 = json.loads([x for x in r1.stdout.splitlines() if x.startswith("{")][0])
+    assert j1["config"]["options"] == 64 and len(j1["kernel_ms_per_slab"]["slabs_of_rank_0"]) == 2
+    assert all(v["lb2"] > 0 for v in j1["kernel_ms_per_slab"]["slabs_of_rank_0"].values())
+    assert all(v["lb2"] == 0 for v in per_slab.values())
