@@ -134,7 +134,7 @@ def lb_two_steps_noalloc(nx, ny, nz, precision, tau, g, f_in, F_lc, f_out, strea
 class Lattice:
     """One lattice on the current CUDA device.  Thin wrapper: every method is one C-ABI call."""
 
-    def __init__(self, nx, ny, nz, tau, device="cuda:0", stream=None, **kw):
+    def __init__(self, nx, ny, nz, tau, device="cuda:0", stream=None, workspace=None, **kw):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2503_06610_b200 needs a CUDA device (no CPU fallback)")
@@ -146,8 +146,13 @@ class Lattice:
             _check(lib.nh_init_lattice(C.byref(self.params), None, 0, None, C.byref(C.c_void_p())))
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-        off = (-self._ws.data_ptr()) % 256
+        if workspace is None:
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            off = (-self._ws.data_ptr()) % 256
+        else:       # the caller's own device memory (uint8 CUDA tensor, 256-byte aligned, >= workspace_bytes)
+            assert workspace.is_cuda and workspace.dtype == torch.uint8 and workspace.is_contiguous()
+            assert workspace.numel() >= nbytes and workspace.data_ptr() % 256 == 0
+            self._ws, off = workspace, 0
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._h = C.c_void_p()
         _check(lib.nh_init_lattice(C.byref(self.params), self._ws.data_ptr() + off, nbytes,
