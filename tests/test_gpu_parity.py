@@ -513,7 +513,8 @@ def test_config3_full_length_invariants():
     eu = rel_linf(out[1]["u"], out[0]["u"])
     en = np.abs(out[1]["n"] - out[0]["n"]).max()
     print("cfg3 20000 steps: FP32 vs FP64 on the GPU rel|du|=%.3e max|dn|=%.3e umax=%.3e" % (eu, en, np.abs(out[0]["u"]).max()))
-    assert eu < 1e-2 and en < 1e-2      # 20x the length north_star gates at 1e-3 / 1e-4; reported, loosely gated
+    # 20x the length north_star gates at 1e-3 / 1e-4; measured 1.9e-3 / 3.9e-3 (deterministic arithmetic: 2x margin)
+    assert eu < 5e-3 and en < 8e-3
 
 
 def test_two_lattices_interleaved_on_two_streams():

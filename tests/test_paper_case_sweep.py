@@ -130,5 +130,5 @@ def test_paper_case_full_model():
     by = {(q["r"], q["prec"]): q for q in rows}
     for r in RATIOS_FULL:
         assert by[(r, "fp64")]["eps_r"] <= 1e-9
-        assert by[(r, "fp32s")]["eps_r"] <= 1e-2
+        assert by[(r, "fp32s")]["eps_r"] <= 1e-3          # measured 5e-7 ... 2e-5 (profiles/r02_paper_case_sweep.md)
         assert by[(r, "fp32s")]["eps_r"] < by[(r, "fp32u")]["eps_r"]
