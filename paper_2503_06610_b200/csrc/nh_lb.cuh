@@ -210,7 +210,7 @@ __device__ __forceinline__ unsigned sweep_block(int reverse) {
   return reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
 }
 
-// One LB step, one thread per fluid cell (baseline variant; nh_lb_vec.cuh holds the wide one).
+// One LB step, one thread per fluid cell (the two-steps-per-launch form is nh_lb2.cuh).
 template <typename T, bool SHIFTED>
 __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 6 : 3)
 lb_step_kernel(const T* __restrict__ fsrc, T* __restrict__ fdst, const T* __restrict__ Flc,
