@@ -47,6 +47,7 @@ extern "C" {
 #define NH_EINVAL  -1   /* null pointer, bad size or parameter                      */
 #define NH_ENOMEM  -2   /* workspace smaller than nh_workspace_bytes()              */
 #define NH_ECUDA   -3   /* a CUDA call failed (including: no device)                */
+#define NH_ENUMERIC -4  /* a non-finite population or director was found (NH_OPT_CHECK_FINITE) */
 
 /* precision */
 #define NH_FP64_SHIFTED    0   /* Eqs. 19-23 in double                                */
@@ -135,7 +136,12 @@ long nh_launch_count(const nh_lattice* L);
  *                        planes >= 256x256, ring <= 48 MB: DESIGN.md section 7).
  *   NH_OPT_LB_ONESTEP    one launch per LB step: neither the two-step kernel nor, on small lattices, the
  *                        cooperative launch that takes all the steps up to the next director update
- * Launch-shape tuning knobs are not part of this contract (include/nh_debug.h).
+ *   NH_OPT_CHECK_FINITE  after the steps of every nh_step call, one more kernel reads the populations and the director
+ *                        (22 words per cell: about half an LB step) and records any NaN or Inf in host-visible memory.
+ *                        Like the wavefront error above this is sticky and asynchronous: the nh_step that produced the
+ *                        value returns NH_OK, every call on the lattice after the kernel has run returns NH_ENUMERIC.
+ *                        For long unattended runs (the paper's are 5e8 steps): call nh_step in chunks.
+ * Launch-shape tuning knobs are not part of this contract (include/nh_debug.h).  Bits not listed here are NH_EINVAL.
  * Setting options resets the timing accumulators. */
 #define NH_OPT_GRAPH          1
 #define NH_OPT_TIMING         2
@@ -144,6 +150,7 @@ long nh_launch_count(const nh_lattice* L);
 #define NH_OPT_FD_NOVEC      32
 #define NH_OPT_LB_TWOSTEP    64
 #define NH_OPT_LB_ONESTEP   128
+#define NH_OPT_CHECK_FINITE 256
 int nh_set_options(nh_lattice* L, int options);
 
 /* Accumulated CUDA-event time (ms) and number of launches of one kernel class since the last

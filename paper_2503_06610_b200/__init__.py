@@ -5,9 +5,9 @@ Only the binding lives here; the kernels are in csrc/ and are compiled by `build
 libnh_b200.so next to this file.  Nothing here imports the CPU oracle.
 """
 from .binding import (FP32_SHIFTED, FP32_UNSHIFTED, FP64_SHIFTED, FP64_UNSHIFTED, KERNEL_CLASSES,
-                      OPT_FD_DIRECT, OPT_FD_NOVEC, OPT_GRAPH, OPT_LB_ONESTEP, OPT_LB_TWOSTEP, OPT_NO_SERPENTINE, OPT_TIMING, TUNE, Lattice, NhError, NhParams,
+                      OPT_CHECK_FINITE, OPT_FD_DIRECT, OPT_FD_NOVEC, OPT_GRAPH, OPT_LB_ONESTEP, OPT_LB_TWOSTEP, OPT_NO_SERPENTINE, OPT_TIMING, TUNE, Lattice, NhError, NhParams,
                       lb_two_steps_noalloc, load, make_params, workspace_bytes)
 
 __all__ = ["Lattice", "NhError", "NhParams", "load", "make_params", "workspace_bytes", "lb_two_steps_noalloc",
            "FP64_SHIFTED", "FP32_SHIFTED", "FP32_UNSHIFTED", "FP64_UNSHIFTED",
-           "OPT_GRAPH", "OPT_TIMING", "OPT_FD_DIRECT", "OPT_NO_SERPENTINE", "OPT_FD_NOVEC", "OPT_LB_TWOSTEP", "OPT_LB_ONESTEP", "KERNEL_CLASSES", "TUNE"]
+           "OPT_GRAPH", "OPT_TIMING", "OPT_FD_DIRECT", "OPT_NO_SERPENTINE", "OPT_FD_NOVEC", "OPT_LB_TWOSTEP", "OPT_LB_ONESTEP", "OPT_CHECK_FINITE", "KERNEL_CLASSES", "TUNE"]

@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(HERE, "libnh_b200.so")
 
 FP64_SHIFTED, FP32_SHIFTED, FP32_UNSHIFTED, FP64_UNSHIFTED = 0, 1, 2, 3
 OPT_GRAPH, OPT_TIMING, OPT_FD_DIRECT, OPT_NO_SERPENTINE, OPT_FD_NOVEC, OPT_LB_TWOSTEP, OPT_LB_ONESTEP = 1, 2, 4, 16, 32, 64, 128
+OPT_CHECK_FINITE = 256
 # keys of nh_debug_tune (include/nh_debug.h: tuning and test hooks, not part of the contract)
 TUNE = {"fd_planes": 0, "lb2_lead": 1, "lb2_ring": 2, "lb2_strips": 3, "lb2_cells": 4, "lb2_threads": 5,
         "lb2_blockorder": 6, "lb2_timeout_ms": 7, "lb2_fault": 8}

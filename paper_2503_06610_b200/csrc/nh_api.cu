@@ -144,6 +144,9 @@ namespace {
 int wave_failed(const nh_lattice* L) {
   if (L->wave_err && *(volatile int*)L->wave_err)
     return fail(NH_ECUDA, "two-step LB kernel: a wavefront dependency wait timed out; the lattice's state is invalid");
+  // (third word of the same host-mapped allocation: set by finite_check_kernel under NH_OPT_CHECK_FINITE)
+  if (L->wave_err && ((volatile int*)L->wave_err)[2])
+    return fail(NH_ENUMERIC, "a population or director component is not finite (NH_OPT_CHECK_FINITE); the lattice's state is invalid");
   return NH_OK;
 }
 
@@ -1012,6 +1015,33 @@ __global__ void rows_kernel(T* __restrict__ field, T* __restrict__ buf, nh::Geom
   else field[at] = buf[to];
 }
 
+// NH_OPT_CHECK_FINITE: one pass over the populations the next step gathers from and over the director; any NaN or Inf
+// sets the host-mapped word that wave_failed() looks at.
+template <typename T>
+__global__ void finite_check_kernel(const T* __restrict__ f, size_t nf, const T* __restrict__ n, size_t nn, int* err) {
+  bool bad = false;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nf + nn; i += stride) {
+    const T v = i < nf ? f[i] : n[i - nf];
+    bad = bad || !isfinite(v);
+  }
+  if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) { *err = 1; __threadfence_system(); }
+}
+template <typename T>
+int launch_finite_check(nh_lattice* L) {
+  Bracket br(L, KC_OTHER);
+  if (br.rc) return br.rc;
+  const size_t nf = 19 * L->G.N, nn = 3 * L->G.N;
+  size_t blocks = (nf + nn + 4 * BLOCK - 1) / (4 * BLOCK);          // four words per thread
+  const size_t most = (size_t)L->sm_count * 16;
+  if (blocks > most) blocks = most;
+  finite_check_kernel<T><<<(unsigned)blocks, BLOCK, 0, L->stream>>>((const T*)L->f[L->cur], nf, (const T*)L->n[L->ncur], nn,
+                                                                   L->wave_err_dev + 2);
+  br.end();
+  NH_CUDA(cudaGetLastError());
+  return NH_OK;
+}
+
 int field_of(nh_lattice* L, int field, void** base, int* comps) {
   switch (field) {
     case NH_FIELD_POPULATIONS: *base = L->f[L->cur]; *comps = 19; return NH_OK;
@@ -1113,9 +1143,9 @@ int nh_init_lattice(const nh_params* p, void* ws, size_t bytes, void* cuda_strea
   L->wave = (unsigned long long*)take(wave_words(p) * 8);
   L->wave_epoch = 0; L->wave_tickets = 0; L->order_key = -1; L->resident_blocks = -1;
   L->wave_err = nullptr;
-  e = cudaHostAlloc((void**)&L->wave_err, 2 * sizeof(int), cudaHostAllocMapped);
+  e = cudaHostAlloc((void**)&L->wave_err, 4 * sizeof(int), cudaHostAllocMapped);
   if (e != cudaSuccess) { delete L; return cuda_fail(e, "cudaHostAlloc(error word)"); }
-  *L->wave_err = 0;
+  L->wave_err[0] = L->wave_err[1] = L->wave_err[2] = L->wave_err[3] = 0;
   L->flag_host = L->wave_err + 1;
   *L->flag_host = 0;
   e = cudaHostGetDevicePointer((void**)&L->wave_err_dev, L->wave_err, 0);
@@ -1174,11 +1204,12 @@ int nh_step(nh_lattice* L, int n_lb, int n_fd) {
   if (n_lb < 0) return fail(NH_EINVAL, "n_lb must be >= 0");
   { const int rc = wave_failed(L); if (rc) return rc; }
   const int r = n_fd < 0 ? L->p.fd_ratio : n_fd;
-  if ((L->options & NH_OPT_GRAPH) && n_lb > 0 && !L->defer_force) {
-    const int rc = step_graph(L, n_lb, r);
-    if (rc != NH_EAGAIN) return rc;          // the stream cannot be captured: plain launches
-  }
-  return step_plain(L, n_lb, r);
+  int rc = NH_EAGAIN;
+  if ((L->options & NH_OPT_GRAPH) && n_lb > 0 && !L->defer_force) rc = step_graph(L, n_lb, r);
+  if (rc == NH_EAGAIN) rc = step_plain(L, n_lb, r);       // (no graphs, or the stream cannot be captured: plain launches)
+  if (rc == NH_OK && (L->options & NH_OPT_CHECK_FINITE) && n_lb > 0)
+    rc = is_f32(L) ? launch_finite_check<float>(L) : launch_finite_check<double>(L);
+  return rc;
 }
 
 int nh_get_fields(nh_lattice* L, double* rho, double* u, double* n, double* F_lc) {
@@ -1262,7 +1293,7 @@ long nh_launch_count(const nh_lattice* L) { return L ? L->launches : -1; }
 int nh_set_options(nh_lattice* L, int options) {
   if (!L) return fail(NH_EINVAL, "null handle");
   constexpr int known = NH_OPT_GRAPH | NH_OPT_TIMING | NH_OPT_FD_DIRECT | NH_OPT_NO_SERPENTINE | NH_OPT_FD_NOVEC |
-                        NH_OPT_LB_TWOSTEP | NH_OPT_LB_ONESTEP;
+                        NH_OPT_LB_TWOSTEP | NH_OPT_LB_ONESTEP | NH_OPT_CHECK_FINITE;
   if (options & ~known) return fail(NH_EINVAL, "unknown option bit (launch-shape knobs moved to nh_debug_tune, include/nh_debug.h)");
   int rc = drain_events(L);
   if (rc) return rc;

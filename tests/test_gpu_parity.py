@@ -310,6 +310,45 @@ def test_options_do_not_change_results():
         assert g.launch_count > 81
 
 
+def test_check_finite_option_reports_a_nan_on_the_next_call():
+    """NH_OPT_CHECK_FINITE: a NaN in the populations (planted through nh_set_rows) is found by the check that follows
+    the steps of nh_step and makes every later call return NH_ENUMERIC; without the option nothing is reported, and a
+    healthy run with the option on is bit-identical to one without."""
+    import torch
+    m = nh()
+    p = I.config(0, fd_ratio=3)
+    d = p.pop("director")
+    p.pop("steps")
+    for precision, dtype in ((1, torch.float32), (0, torch.float64)):
+        ref = m.Lattice(**dict(p, precision=precision))
+        ref.set_director(d)
+        ref.step(12)
+        g = m.Lattice(**dict(p, precision=precision))
+        g.set_options(m.OPT_CHECK_FINITE)
+        g.set_director(d)
+        for _ in range(4):
+            g.step(3)
+        fr, fg = ref.get_fields(), g.get_fields()               # no error, same bits
+        for k in fr:
+            assert np.array_equal(fr[k], fg[k]), k
+        for lat, checked in ((ref, False), (g, True)):
+            rows = lat.new_rows_buffer("populations", 1)
+            lat.get_rows("populations", 5, 1, rows)
+            rows.view(dtype)[p["nx"] * 1 + 7] = float("nan")       # rest population of the cell (7, 5, 1): a fluid cell
+            lat.set_rows("populations", 5, 1, rows)
+            lat.step(2)                                          # asynchronous: this call cannot know yet
+            lat.synchronize()
+            if checked:
+                for call in (lambda: lat.step(1), lambda: lat.get_fields(), lambda: lat.update_force()):
+                    with pytest.raises(m.NhError) as ei:
+                        call()
+                    assert ei.value.code == -4 and "not finite" in str(ei.value)
+            else:
+                lat.step(1)
+                assert not np.isfinite(lat.get_fields(which=("u",))["u"]).all()
+            lat.close()
+
+
 def test_unknown_option_bits_are_refused_and_option_changes_drop_graphs():
     """nh_set_options: bits that are not in include/nh.h (the launch-shape bits of earlier builds, now nh_debug_tune
     keys) are NH_EINVAL and leave the options as they were; switching a kernel-selecting bit while graphs are held
@@ -321,7 +360,7 @@ def test_unknown_option_bits_are_refused_and_option_changes_drop_graphs():
     p.pop("steps")
     g = m.Lattice(stream=torch.cuda.Stream(), **dict(p, precision=0))
     g.set_options(m.OPT_GRAPH)
-    for bad in (8, 1 << 26, 1 << 8, m.OPT_GRAPH | (1 << 30)):
+    for bad in (8, 1 << 26, 1 << 9, m.OPT_GRAPH | (1 << 30)):
         with pytest.raises(m.NhError) as ei:
             g.set_options(bad)
         assert ei.value.code == -1 and "unknown option bit" in str(ei.value)
