@@ -135,3 +135,28 @@ def test_no_alloc_entry_validates_before_it_touches_cuda(lib):
         has_gpu = False
     if not has_gpu:
         assert call(64, 8, 6, 1, 0.8) == -3 and lib.nh_last_error()
+
+
+def test_binding_constants_equal_the_headers():
+    """Every #define of the headers that the binding mirrors has the same value there: options, precisions, fields,
+    tuning keys, error codes, the no-alloc scratch size."""
+    defs = {}
+    for header in ("nh.h", "nh_debug.h", "nh_noalloc.h"):
+        text = open(os.path.join(ROOT, "include", header)).read()
+        for name, value in re.findall(r"^#define\s+(NH_[A-Z0-9_]+)\s+(\(?[-0-9ux* ]+\)?)", text, flags=re.M):
+            defs[name] = eval(value.replace("u", ""))          # plain integer expressions: 16u * 1024u * 1024u
+    b = nh.binding
+    for name in ("GRAPH", "TIMING", "FD_DIRECT", "NO_SERPENTINE", "FD_NOVEC", "LB_TWOSTEP", "LB_ONESTEP", "CHECK_FINITE"):
+        assert getattr(b, "OPT_" + name) == defs["NH_OPT_" + name], name
+    for name in ("FP64_SHIFTED", "FP32_SHIFTED", "FP32_UNSHIFTED", "FP64_UNSHIFTED"):
+        assert getattr(b, name) == defs["NH_" + name], name
+    for i, field in enumerate(b.FIELDS):
+        assert defs["NH_FIELD_" + field.upper()] == i
+    for key, value in b.TUNE.items():
+        assert defs["NH_TUNE_" + key.upper()] == value, key
+    assert len(b.TUNE) == defs["NH_TUNE_COUNT"]
+    assert b.NOALLOC_SCRATCH_BYTES == defs["NH_NOALLOC_SCRATCH_BYTES"] == 16 * 1024 * 1024
+    assert (defs["NH_OK"], defs["NH_EINVAL"], defs["NH_ENOMEM"], defs["NH_ECUDA"], defs["NH_ENUMERIC"]) == (0, -1, -2, -3, -4)
+    # option bits are distinct single bits
+    bits = [v for k, v in defs.items() if k.startswith("NH_OPT_")]
+    assert len(set(bits)) == len(bits) and all(v & (v - 1) == 0 for v in bits)
