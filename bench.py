@@ -10,7 +10,10 @@ One bench "step" is one pass over every row of the hot path: r LB steps (collide
 then the velocity store, predictor, corrector and force update.  MLUPS = fluid cells x LB steps /
 seconds / 1e6 (reading G21).
 
-Prints ONE JSON line (rank 0).  Multi-GPU (--gpus N, under torchrun or started by bench.py itself): ONE lattice of N
+Prints ONE JSON line (rank 0).  Beyond the contract's keys: `roofline` (dominant LB kernel: `bound` "hbm" for the one-step
+kernels, "latency" for the two-step kernel with `own_dram_floor_frac`, its time against one pass over HBM per pair of steps),
+`sustained` (the same loop for >= 3 s: clocks, power, `mlups_per_watt`), `fp64` and `one_step` sub-records, `e2e` through
+the C ABI with pinned host buffers, `cpu_baseline` (the oracle on the host cores).  Both arms take `config` from config_of().  Multi-GPU (--gpus N, under torchrun or started by bench.py itself): ONE lattice of N
 times the config's rows, cut into N y-slabs, one per rank, halo rows exchanged over NCCL (weak scaling; DESIGN.md
 section 8); --replicas runs N independent lattices instead.
 """
